@@ -1,0 +1,438 @@
+"""Pins of the oracle (oracle/mhd_oracle.cpp) to things OTHER than itself  (-m "not gpu").
+
+The paper prints no numerical field values (figures only), so the pins are what the paper and the
+mathematics fix: conservation (flux form), div B (constrained transport), second
+order in space and time measured on linear MHD eigenmodes against their closed-form
+solution, the exact Riemann solution for B = 0, symmetries, exact special cases, and a brute-force
+comparison with an independently structured NumPy restatement on tiny grids.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_0908_4362_b200 import inputs
+from tests import np_restatement as npr
+
+P, O = inputs.PERIODIC, inputs.OUTFLOW
+
+
+def c64(fields):
+    return [np.array(f, dtype=np.float64, order="C", copy=True) for f in fields]   # never aliased
+
+
+def divb(f, bc=P):
+    """discrete div B in grid units (SURVEY.md pin P2); last cell of an outflow axis excluded by caller"""
+    sp = lambda a, ax: inputs._shift_plus(a, ax, bc)
+    return (sp(f[5], 2) - f[5]) + (sp(f[6], 1) - f[6]) + (sp(f[7], 0) - f[7])
+
+
+def ksum(a):
+    return math.fsum(a.ravel().tolist())
+
+
+# ---------------------------------------------------------------------------------------------
+# P1 / P2: conservation and div B
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", ["ot64", "turb3d"])
+def test_conservation_and_divb_periodic(case):
+    if case == "ot64":
+        f, meta = inputs.orszag_tang(64)
+        nsteps = 30
+    else:
+        f, meta = inputs.turbulence(24, 20, 16)
+        nsteps = 6
+    f = c64(f)
+    assert np.abs(divb(f)).max() <= 1e-13 * max(np.abs(f[5]).max(), np.abs(f[6]).max(), np.abs(f[7]).max()) * 64
+    s0 = [ksum(a) for a in f]
+    a0 = [ksum(np.abs(a)) for a in f]
+    oracle.run(f, meta["gamma"], meta["bc"], 0, nsteps, 0.8)
+    s1 = [ksum(a) for a in f]
+    for name, x0, x1, sc in zip(inputs.FIELD_NAMES, s0, s1, a0):
+        if sc > 0:
+            assert abs(x1 - x0) <= 1e-13 * sc, (name, x0, x1)
+        else:
+            assert x1 == 0.0, name
+    bmax = max(np.abs(f[5]).max(), np.abs(f[6]).max(), np.abs(f[7]).max())
+    assert np.abs(divb(f)).max() <= 1e-12 * bmax
+    assert f[0].min() > 0
+
+
+def test_divb_outflow_interior():
+    f, meta = inputs.turbulence(16, 12, 10)
+    f = c64(f)
+    oracle.run(f, meta["gamma"], O, 0, 4, 0.8)
+    dv = divb(f, O)[:-1, :-1, :-1]      # the +face of the last cell is the clamped copy (reading R9)
+    assert np.abs(dv).max() <= 1e-12 * np.abs(f[5]).max()
+
+
+# ---------------------------------------------------------------------------------------------
+# P3: linear MHD eigenmodes along x -- closed-form solution, second-order convergence
+# ---------------------------------------------------------------------------------------------
+V0 = 0.3   # background flow along x: keeps v_x away from 0, where |v_x| in the freezing speed
+           # puts a kink into the right/left-going split and the measured order of
+           # compressive modes drops to ~1.5 ("What the pins found")
+
+
+def _eigenmode(kind, n, eps, phase_shift=0.0):
+    """Right-going plane-wave eigenmode of linearised ideal MHD about rho=1, p=1, B=(1,1,0.5), v=(V0,0,0).
+
+    Linearising eqs (1)-(4) PAPER.md:51-62 for f(x - c t):  dvx = c e, dp = gamma p e, drho = rho e,
+    dB_perp = B_perp c^2 e / (c^2 - ca^2), dv_perp = -bx dB_perp / (rho c); c solves
+    (c^2 - a^2)(c^2 - ca^2) = c^2 ct^2 (fast/slow); Alfven: c = ca, dB_perp orthogonal to B_perp.
+    Returns (fields for the given phase shift, pattern speed V0 + c, gamma).
+    """
+    gamma = 5.0 / 3.0
+    rho0, p0, bx, by, bz = 1.0, 1.0, 1.0, 1.0, 0.5
+    a2, ca2, ct2 = gamma * p0 / rho0, bx * bx / rho0, (by * by + bz * bz) / rho0
+    s = a2 + ca2 + ct2
+    disc = math.sqrt(s * s - 4 * a2 * ca2)
+    xc = np.arange(n) + 0.5
+    e = eps * np.sin(2 * math.pi * (xc - phase_shift) / n)
+    if kind == "alfven":
+        c = math.sqrt(ca2)
+        nb = math.hypot(by, bz)
+        dby, dbz = e * (-bz / nb), e * (by / nb)
+        drho, dvx, dp = 0 * e, V0 + 0 * e, 0 * e
+    else:
+        c2 = 0.5 * (s + disc) if kind == "fast" else 0.5 * (s - disc)
+        c = math.sqrt(c2)
+        drho, dvx, dp = rho0 * e, V0 + c * e, gamma * p0 * e
+        dby, dbz = by * c2 * e / (c2 - ca2), bz * c2 * e / (c2 - ca2)
+    dvy, dvz = -bx * dby / (rho0 * c), -bx * dbz / (rho0 * c)
+    shape = (1, 1, n)
+    rho = (rho0 + drho).reshape(shape)
+    vx, vy, vz = dvx.reshape(shape), dvy.reshape(shape), dvz.reshape(shape)
+    p = (p0 + dp).reshape(shape)
+    Bx = np.full(shape, bx)
+    By, Bz = (by + dby).reshape(shape), (bz + dbz).reshape(shape)   # transverse faces sit at the x centre
+    E = inputs.total_energy(rho, vx, vy, vz, p, Bx, By, Bz, gamma, P)
+    return c64([rho, rho * vx, rho * vy, rho * vz, E, Bx, By, Bz]), V0 + c, gamma
+
+
+@pytest.mark.parametrize("kind", ["alfven", "fast", "slow"])
+def test_eigenmode_second_order_convergence(kind):
+    eps = 1e-6
+    errs = []
+    sizes = [32, 64, 128, 256]
+    for n in sizes:
+        f, c, gamma = _eigenmode(kind, n, eps)
+        cm = oracle.cmax(f, gamma, P)
+        t_end = n / c                                  # one period in grid units
+        nsteps = math.ceil(t_end / (2 * 0.8 / cm))
+        dt = t_end / (2 * nsteps)
+        for s in range(nsteps):
+            oracle.step_fixed(f, gamma, P, s, dt)
+        ref, _, _ = _eigenmode(kind, n, eps, phase_shift=c * t_end)
+        err = sum(np.abs(a - b).mean() for a, b in zip(f, ref)) / eps
+        errs.append(err)
+    orders = [math.log2(errs[i] / errs[i + 1]) for i in range(len(errs) - 1)]
+    # a dropped or mis-signed flux term gives a wrong wave speed: O(1) error and no convergence
+    assert errs[-1] < 8e-3, (errs, orders)
+    assert all(o > 1.7 for o in orders), (errs, orders)
+    assert orders[-1] > 1.9, (errs, orders)
+
+
+def test_eigenmode_travels_at_wave_speed_not_half_period():
+    """After HALF a period the fast mode must match the half-shifted profile and NOT the initial one."""
+    n, eps = 128, 1e-6
+    f, c, gamma = _eigenmode("fast", n, eps)
+    cm = oracle.cmax(f, gamma, P)
+    t_end = 0.5 * n / c
+    nsteps = math.ceil(t_end / (2 * 0.8 / cm))
+    for s in range(nsteps):
+        oracle.step_fixed(f, gamma, P, s, t_end / (2 * nsteps))
+    moved, _, _ = _eigenmode("fast", n, eps, phase_shift=c * t_end)
+    still, _, _ = _eigenmode("fast", n, eps)
+    e_moved = sum(np.abs(a - b).mean() for a, b in zip(f, moved)) / eps
+    e_still = sum(np.abs(a - b).mean() for a, b in zip(f, still)) / eps
+    assert e_moved < 0.03 and e_still > 1.0, (e_moved, e_still)
+
+
+# ---------------------------------------------------------------------------------------------
+# B = 0: exact Riemann solution of the Euler equations (Sod tube), textbook closed form
+# ---------------------------------------------------------------------------------------------
+def _sod_exact(x, t, gamma=1.4, left=(1.0, 0.0, 1.0), right=(0.125, 0.0, 0.1), x0=0.5):
+    rl, ul, pl = left
+    rr, ur, pr = right
+    g = gamma
+    al, ar = math.sqrt(g * pl / rl), math.sqrt(g * pr / rr)
+
+    def fk(p, rk, pk, ak):
+        if p > pk:   # shock
+            A, B = 2 / ((g + 1) * rk), (g - 1) / (g + 1) * pk
+            return (p - pk) * math.sqrt(A / (p + B))
+        return 2 * ak / (g - 1) * ((p / pk) ** ((g - 1) / (2 * g)) - 1)
+
+    lo, hi = 1e-8, 10.0
+    for _ in range(200):   # bisection on f(p) = fL + fR + (uR - uL)
+        mid = 0.5 * (lo + hi)
+        if fk(mid, rl, pl, al) + fk(mid, rr, pr, ar) + (ur - ul) > 0:
+            hi = mid
+        else:
+            lo = mid
+    ps = 0.5 * (lo + hi)
+    us = 0.5 * (ul + ur) + 0.5 * (fk(ps, rr, pr, ar) - fk(ps, rl, pl, al))
+    # left rarefaction, right shock (Sod)
+    rsl = rl * (ps / pl) ** (1 / g)
+    asl = al * (ps / pl) ** ((g - 1) / (2 * g))
+    rsr = rr * ((ps / pr + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * ps / pr + 1))
+    S = ur + ar * math.sqrt((g + 1) / (2 * g) * ps / pr + (g - 1) / (2 * g))
+    xi = (x - x0) / t
+    rho = np.empty_like(x)
+    head, tail = ul - al, us - asl
+    for i, s in enumerate(xi):
+        if s < head:
+            rho[i] = rl
+        elif s < tail:
+            rho[i] = rl * (2 / (g + 1) + (g - 1) / ((g + 1) * al) * (ul - s)) ** (2 / (g - 1))
+        elif s < us:
+            rho[i] = rsl
+        elif s < S:
+            rho[i] = rsr
+        else:
+            rho[i] = rr
+    return rho
+
+
+def test_sod_tube_against_exact_riemann_solution():
+    gamma, t_phys = 1.4, 0.2
+    errs = []
+    for n in (100, 200, 400):
+        x = (np.arange(n) + 0.5) / n
+        shape = (1, 1, n)
+        rho = np.where(x < 0.5, 1.0, 0.125).reshape(shape)
+        p = np.where(x < 0.5, 1.0, 0.1).reshape(shape)
+        z = np.zeros(shape)
+        f = c64([rho, z, z, z, p / (gamma - 1), z, z, z])
+        t, s = 0.0, 0
+        t_end = t_phys * n
+        while t < t_end - 1e-12:
+            dt = min(0.8 / oracle.cmax(f, gamma, O), 0.5 * (t_end - t))
+            oracle.step_fixed(f, gamma, O, s, dt)
+            t += 2 * dt
+            s += 1
+        for b in f[5:]:
+            assert not b.any()                       # B stays bitwise zero (pin P9)
+        exact = _sod_exact(x, t_phys, gamma)
+        errs.append(np.abs(f[0].ravel() - exact).mean())
+    assert errs[0] < 1.2e-2 and errs[2] < 4e-3, errs
+    assert errs[1] < 0.75 * errs[0] and errs[2] < 0.75 * errs[1], errs     # converging (first order at shocks)
+
+
+# ---------------------------------------------------------------------------------------------
+# P4: Orszag-Tang 180-degree rotation symmetry
+# ---------------------------------------------------------------------------------------------
+def test_orszag_tang_rotation_symmetry():
+    n = 64
+    f, meta = inputs.orszag_tang(n)
+    f = c64(f)
+    oracle.run(f, meta["gamma"], meta["bc"], 0, 30, 0.8)
+    rot = lambda a: a[:, ::-1, ::-1]
+    scale = np.abs(f[4]).max()
+    assert np.abs(rot(f[0]) - f[0]).max() <= 1e-10 * scale
+    assert np.abs(rot(f[4]) - f[4]).max() <= 1e-10 * scale
+    assert np.abs(rot(f[1]) + f[1]).max() <= 1e-10 * scale
+    assert np.abs(rot(f[2]) + f[2]).max() <= 1e-10 * scale
+    # faces: Bx[i,j] at (i-1/2, j) maps to ((n-i) mod n, n-1-j)
+    bx, by = f[5][0], f[6][0]
+    i = np.arange(n)
+    bxr = bx[np.ix_(n - 1 - i, (n - i) % n)]          # [j', i'] = [n-1-j, (n-i)%n]
+    byr = by[np.ix_((n - i) % n, n - 1 - i)]
+    assert np.abs(bxr + bx).max() <= 1e-10
+    assert np.abs(byr + by).max() <= 1e-10
+    assert np.abs(bx).max() > 0.1
+
+
+# ---------------------------------------------------------------------------------------------
+# P5 / P6 / P7: exact special cases
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [P, O])
+def test_uniform_state_is_a_bitwise_fixed_point(bc):
+    shape = (5, 6, 7)
+    vals = [1.3, 0.4, -0.7, 0.2, 3.1, 0.6, -0.3, 0.9]
+    f = [np.full(shape, v) for v in vals]
+    g = [a.copy() for a in f]
+    for s in range(3):
+        oracle.step_fixed(g, 5.0 / 3.0, bc, s, 0.37)
+    for a, b in zip(f, g):
+        assert np.array_equal(a, b)
+
+
+def test_1d_data_replicated_in_3d_is_bitwise_1d():
+    f1, meta = inputs.brio_wu(64)
+    f1 = c64(f1)
+    f3 = c64([np.broadcast_to(a, (4, 4, 64)) for a in f1])
+    for s in range(4):
+        oracle.step_fixed(f1, meta["gamma"], meta["bc"], s, 0.2)
+        oracle.step_fixed(f3, meta["gamma"], meta["bc"], s, 0.2)
+    for a, b in zip(f1, f3):
+        assert np.array_equal(np.broadcast_to(a, b.shape), b)
+
+
+def _cyclic(f):
+    """x->y->z->x: new field(y=a, z=b, x=c) = old field(x=a, y=b, z=c); vector components follow."""
+    tr = lambda a: np.ascontiguousarray(a.transpose(1, 2, 0))    # new[z,y,x] = old[k=y', ...]
+    # old array index order (z,y,x); new axes: new_x = old_z, new_y = old_x, new_z = old_y
+    # new[z',y',x'] = old[z=x', y=z', x=y']  -> transpose(1,2,0) of old gives axes (y,x,z) -> indices [z'=y, y'=x, x'=z]
+    rho, mx, my, mz, E, bx, by, bz = f
+    return [tr(rho), tr(mz), tr(mx), tr(my), tr(E), tr(bz), tr(bx), tr(by)]
+
+
+@pytest.mark.parametrize("bc", [P, O])
+def test_cyclic_permutation_equivariance_bitwise(bc):
+    f, meta = inputs.turbulence(12, 10, 8)
+    f = c64(f)
+    g = _cyclic(f)                      # axes rotated: old x-direction is the new y-direction
+    for s in range(3):
+        oracle.step_fixed(f, meta["gamma"], bc, s, 0.11)
+        # old order (x,y,z) at s=0 is (y,z,x) in the new frame = the table row for s+2
+        oracle.step_fixed(g, meta["gamma"], bc, s + 2, 0.11)
+    for a, b in zip(_cyclic(f), g):
+        assert np.array_equal(a, b)
+
+
+def test_thread_count_does_not_change_bits():
+    f, meta = inputs.turbulence(16, 12, 10)
+    a, b = c64(f), c64(f)
+    n0 = oracle.num_threads()
+    try:
+        oracle.set_num_threads(1)
+        oracle.run(a, meta["gamma"], meta["bc"], 0, 2, 0.8)
+        oracle.set_num_threads(max(2, n0))
+        oracle.run(b, meta["gamma"], meta["bc"], 0, 2, 0.8)
+    finally:
+        oracle.set_num_threads(n0)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+# ---------------------------------------------------------------------------------------------
+# P8: Brio-Wu invariants and qualitative wave structure
+# ---------------------------------------------------------------------------------------------
+def _run_to(f, meta, t_end_grid, cfl=0.8):
+    t, s = 0.0, 0
+    while t < t_end_grid - 1e-12:
+        dt = min(cfl / oracle.cmax(f, meta["gamma"], meta["bc"]), 0.5 * (t_end_grid - t))
+        oracle.step_fixed(f, meta["gamma"], meta["bc"], s, dt)
+        t += 2 * dt
+        s += 1
+    return s
+
+
+def test_brio_wu_invariants_and_structure():
+    n = 512
+    f, meta = inputs.brio_wu(n)
+    f = c64(f)
+    nsteps = _run_to(f, meta, 0.1 * n)
+    assert 100 < nsteps < 200
+    rho, mx, my, mz, E, bx, by, bz = [a.ravel() for a in f]
+    assert np.all(bx == 0.75) and not mz.any() and not bz.any()
+    b2 = bx ** 2 + (0.5 * (by + by)) ** 2
+    p = (meta["gamma"] - 1) * (E - 0.5 * (mx ** 2 + my ** 2) / rho - 0.5 * b2)
+    assert rho.min() > 0 and p.min() > 0
+    # undisturbed end states
+    assert abs(rho[5] - 1.0) < 1e-12 and abs(rho[-5] - 0.125) < 1e-12
+    assert abs(by[5] - 1.0) < 1e-12 and abs(by[-5] + 1.0) < 1e-12
+    # By goes from +1 to -1; fluid is pushed to the right in the middle (vx > 0), v_y < 0
+    assert by[n // 4] > 0 > by[3 * n // 4]
+    assert (mx / rho).max() > 0.5 and (my / rho).min() < -1.0
+    # density: left rarefaction fan (monotone decreasing), and somewhere a dip below the right state
+    # (right-going fast rarefaction), and an intermediate plateau between 0.6 and 0.75
+    x = (np.arange(n) + 0.5) / n
+    fan = rho[(x > 0.33) & (x < 0.42)]
+    assert np.all(np.diff(fan) < 0)
+    assert rho.min() < 0.125 - 1e-3
+    plateau = rho[(x > 0.50) & (x < 0.54)]
+    assert 0.6 < plateau.mean() < 0.75
+
+
+# ---------------------------------------------------------------------------------------------
+# P10: the scalar B advection scheme with constant velocity on linear data is exact
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("d,t", [(0, 1), (0, 2), (1, 2), (1, 0), (2, 0), (2, 1)])
+@pytest.mark.parametrize("v", [0.7, -0.45])
+def test_badvect_constant_velocity_linear_data_exact(d, t, v):
+    n = [9, 10, 11]
+    shape = (n[2], n[1], n[0])
+    slope, dt = 0.25, 0.6
+    idx = np.arange(n[d], dtype=np.float64)
+    bshape = [1, 1, 1]
+    bshape[2 - d] = n[d]
+    lin = np.broadcast_to((slope * idx).reshape(bshape), shape)
+    f = [np.ones(shape), np.zeros(shape), np.zeros(shape), np.zeros(shape), np.full(shape, 10.0),
+         np.zeros(shape), np.zeros(shape), np.zeros(shape)]
+    f[1 + d] = np.full(shape, v)
+    f[5 + t] = lin.copy()
+    f[5 + d] = np.full(shape, 0.3)
+    f = c64(f)
+    oracle.badvect(f, 5.0 / 3.0, P, d, t, dt)
+    sl = [slice(None)] * 3
+    sl[2 - d] = slice(3, n[d] - 3)          # away from the wrap-around jump of the linear profile
+    got = f[5 + t][tuple(sl)]
+    want = (lin - v * dt * slope)[tuple(sl)]
+    assert np.abs(got - want).max() < 1e-14
+    assert np.abs(f[5 + d][tuple(sl)] - 0.3).max() < 1e-15     # same flux on every row: no constraint change
+    s = 3 - d - t
+    assert np.array_equal(f[5 + s], np.zeros(shape))
+
+
+# ---------------------------------------------------------------------------------------------
+# P11: brute force on tiny grids against the independently structured NumPy restatement
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape", [(4, 1, 1), (1, 5, 1), (1, 1, 4), (4, 4, 1), (4, 3, 2), (7, 5, 6), (2, 2, 2)])
+@pytest.mark.parametrize("bc", [P, O])
+def test_tiny_grids_against_numpy_restatement(shape, bc):
+    nx, ny, nz = shape
+    rng = np.random.default_rng(nx * 100 + ny * 10 + nz + bc)
+    sh = (nz, ny, nx)
+    rho = 1.0 + 0.3 * rng.random(sh)
+    v = [0.5 * rng.standard_normal(sh) for _ in range(3)]
+    B = [0.5 * rng.standard_normal(sh) for _ in range(3)]
+    E = 2.5 + rng.random(sh) + 0.5 * rho * sum(x * x for x in v) + sum(x * x for x in B)
+    f0 = c64([rho, rho * v[0], rho * v[1], rho * v[2], E] + B)
+    gamma, dt = 5.0 / 3.0, 0.13
+    assert abs(oracle.cmax(f0, gamma, bc) - npr.cmax(f0, gamma, bc)) < 1e-14
+    for d in range(3):
+        a = [x.copy() for x in f0]
+        oracle.fluid(a, gamma, bc, d, dt)
+        b = npr.fluid(f0, gamma, bc, d, dt)
+        for x, y in zip(a, b):
+            assert np.abs(x - y).max() < 1e-13
+        for t in range(3):
+            if t == d:
+                continue
+            a = [x.copy() for x in f0]
+            oracle.badvect(a, gamma, bc, d, t, dt)
+            b = npr.badvect(f0, gamma, bc, d, t, dt)
+            for x, y in zip(a, b):
+                assert np.abs(x - y).max() < 1e-13
+    for s in range(3):
+        a = [x.copy() for x in f0]
+        oracle.step_fixed(a, gamma, bc, s, dt)
+        b = npr.step(f0, gamma, bc, s, dt)
+        for x, y in zip(a, b):
+            assert np.abs(x - y).max() < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# P12: fp32 instantiation sanity (same magnitudes as PAPER.md:567-583)
+# ---------------------------------------------------------------------------------------------
+def test_fp32_oracle_tracks_fp64_oracle():
+    f, meta = inputs.brio_wu(512)
+    a = inputs.to_precision(f, np.float64)
+    b = inputs.to_precision(f, np.float32)
+    for s in range(40):
+        dt = 0.8 / oracle.cmax(a, meta["gamma"], meta["bc"])
+        oracle.step_fixed(a, meta["gamma"], meta["bc"], s, dt)
+        oracle.step_fixed(b, meta["gamma"], meta["bc"], s, dt)
+    for x, y in zip(a, b):
+        assert np.abs(x - y).max() < 2e-5      # paper: <= 1e-6-ish for Brio-Wu at t = 0.08
+
+
+def test_cmax_surfaces_nan():
+    f, meta = inputs.turbulence(8, 8, 8)
+    f = c64(f)
+    f[0][3, 3, 3] = np.nan
+    assert math.isnan(oracle.cmax(f, meta["gamma"], meta["bc"]))
