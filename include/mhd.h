@@ -1,0 +1,132 @@
+/* mhd.h -- C ABI of libmhd.so: the per-timestep update of the 3-D ideal-MHD conserved state by the
+ * second-order relaxing-TVD scheme of arxiv/paper_0908_4362 (section 3, lines 47-172),
+ * hand-written for NVIDIA B200 (sm_100a).  The calls follow the paper's program flow
+ * (PAPER.md:233-243): initial u on cells and B on faces in; loop { c_max -> dt; six L_i; t += 2 dt };
+ * state out.
+ *
+ * Conventions
+ *   - Plain C.  No exception crosses this boundary and the library never calls exit().  Every call
+ *     that returns int returns MHD_OK (0) or a negative mhd_status; the message of the last failure
+ *     of a context is available from mhd_last_error().
+ *   - Grid units: cells have unit width; dt, t and all speeds are in cells per unit
+ *     time.  For a unit box of n cells t_physical = t_grid / n.
+ *   - State: eight fields in the order rho, m_x, m_y, m_z, E, Bx, By, Bz, each a
+ *     dense array of N = nx*ny*nz elements of the context's precision, x fastest:
+ *         idx = i + nx*(j + ny*k).
+ *     u = (rho, m, E) is cell centred; B is face centred (eq (19)):
+ *     Bx[i,j,k] = B_x at (i-1/2,j,k), By[i,j,k] = B_y at (i,j-1/2,k), Bz[i,j,k] = B_z at (i,j,k-1/2).
+ *   - Boundary rule (the paper is silent; reading R9): every read of an operator's input at
+ *     an out-of-range index is mapped by wrap (MHD_BC_PERIODIC) or clamp (MHD_BC_OUTFLOW), the same
+ *     rule on all three axes.
+ *   - One step = one c_max reduction + one double sweep of six L_i operators with the rotation of
+ *     eqs (23)-(25), advancing t by 2 dt.
+ *   - Ownership: the context owns (or, after mhd_bind, borrows) all device memory.  set/get copy; the
+ *     caller keeps every pointer it passes and none needs to outlive the call.
+ *   - Pointers are HOST pointers unless the argument says otherwise ("where" = MHD_DEVICE).
+ *   - All work is enqueued on the context's CUDA stream; calls marked "synchronises" wait for it.
+ *   - Not thread safe per context; distinct contexts are independent.
+ */
+#ifndef MHD_H_
+#define MHD_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mhd_ctx mhd_ctx; /* opaque, owned by the library */
+
+enum mhd_precision { MHD_F32 = 0, MHD_F64 = 1 };
+enum mhd_bc { MHD_BC_PERIODIC = 0, MHD_BC_OUTFLOW = 1 };
+enum mhd_where { MHD_HOST = 0, MHD_DEVICE = 1 };
+enum mhd_status {
+  MHD_OK = 0,
+  MHD_EINVAL = -1,     /* bad argument: extent < 1, gamma <= 1, unknown enum, NULL pointer, cfl <= 0, n < 0 */
+  MHD_ENOMEM = -2,     /* allocation failed, or mhd_bind workspace too small / misaligned */
+  MHD_ECUDA = -3,      /* a CUDA call failed (message in mhd_last_error) */
+  MHD_ENONFINITE = -4, /* the c_max reduction saw NaN/Inf or c_max <= 0 (state is poisoned) */
+  MHD_ENOSTATE = -5    /* stepping or reading before mhd_set_state */
+};
+enum mhd_operator { MHD_OP_FLUID = 0, MHD_OP_BPAIR = 1, MHD_OP_SWEEP_FORWARD = 2, MHD_OP_SWEEP_REVERSE = 3 };
+
+/* Bytes of device memory a context of this shape needs (two copies of the 8 fields for out-of-place
+ * operators plus a small scalar block).  Returns 0 on invalid arguments. */
+size_t mhd_workspace_bytes(int nx, int ny, int nz, int precision);
+
+/* Create a context for an nx*ny*nz grid (any extents >= 1; an extent of 1 makes that axis
+ * degenerate, e.g. 512x1x1 for 1-D runs).  gamma > 1 is the adiabatic index of
+ * P = (gamma-1)(E - rho v^2/2 - B^2/2).  No device memory is touched until the first
+ * call that needs it (mhd_bind or mhd_set_state).  *out receives the context. */
+int mhd_create(int nx, int ny, int nz, double gamma, int precision, int bc, mhd_ctx** out);
+
+/* Optional.  Use caller-owned DEVICE memory (at least mhd_workspace_bytes, 256-byte aligned) and/or a
+ * caller-owned CUDA stream (a cudaStream_t passed as void*; NULL = the default stream) instead of
+ * the library's own cudaMalloc / own stream.  Must precede mhd_set_state.  The memory is borrowed
+ * until mhd_destroy.  device_workspace == NULL keeps library-owned memory and only sets the stream. */
+int mhd_bind(mhd_ctx* ctx, void* device_workspace, size_t bytes, void* cuda_stream);
+
+/* Free the context and everything it owns.  Synchronises.  NULL is allowed. */
+int mhd_destroy(mhd_ctx* ctx);
+
+/* Copy a full state IN.  fields[0..7] point to N elements each of the context's precision, in host
+ * (where = MHD_HOST, pageable or pinned) or device (MHD_DEVICE) memory.  Resets the time
+ * accumulated by the context to 0 but not the step index.  Synchronises for host sources. */
+int mhd_set_state(mhd_ctx* ctx, const void* const fields[8], int where);
+
+/* Copy the current state OUT into fields[0..7] (N elements each).  Synchronises. */
+int mhd_get_state(mhd_ctx* ctx, void* const fields[8], int where);
+
+/* c_max of eq (18) (B interpolated to cell centres) and dt = cfl / c_max, in grid
+ * units.  Writes dt to *dt_out and, if cmax_out != NULL, c_max to *cmax_out.  Synchronises.
+ * MHD_ENONFINITE if c_max is NaN, Inf or <= 0. */
+int mhd_cfl_dt(mhd_ctx* ctx, double cfl, double* dt_out, double* cmax_out);
+
+/* n steps (n >= 0), each: c_max reduction, dt = cfl / c_max kept on the device, six L_i with that
+ * dt, step index += 1, t += 2 dt.  If t_advanced != NULL the call synchronises,
+ * writes the time advanced by THIS call and reports MHD_ENONFINITE if any reduction was poisoned;
+ * if it is NULL nothing is read back and the call returns as soon as the work is enqueued. */
+int mhd_step(mhd_ctx* ctx, int n, double cfl, double* t_advanced);
+
+/* n steps with the caller's dt (> 0, grid units) instead of the CFL value; no reduction is run.
+ * Used for parity tests and for clipping the last step to a target time.  Does not synchronise. */
+int mhd_step_fixed(mhd_ctx* ctx, int n, double dt);
+
+/* One operator of the step, for per-operator parity tests: op = MHD_OP_FLUID (fluid_d, Algorithm 1,
+ * PAPER.md:273-285), MHD_OP_BPAIR (B_{t1->d} then B_{t2->d}, or t2 then t1 if reverse != 0;
+ * Algorithm 2), MHD_OP_SWEEP_FORWARD / MHD_OP_SWEEP_REVERSE (L_d, PAPER.md:162,
+ * 317; `reverse` is ignored).  d = 0, 1, 2 for x, y, z.  Does not synchronise. */
+int mhd_apply(mhd_ctx* ctx, int op, int d, int reverse, double dt);
+
+/* Step index s selects the sweep order (x,y,z), (z,x,y), (y,z,x) for s mod 3 = 0, 1, 2. */
+int mhd_get_step_index(mhd_ctx* ctx, long long* s);
+int mhd_set_step_index(mhd_ctx* ctx, long long s);
+
+/* Total time advanced since the last mhd_set_state (grid units).  Synchronises. */
+int mhd_get_time(mhd_ctx* ctx, double* t);
+
+/* Not on the timed path.  sums[0..7] = sum over cells of each field (double accumulation);
+ * *max_abs_divb = max |(Bx[i+1]-Bx[i]) + (By[j+1]-By[j]) + (Bz[k+1]-Bz[k])| over cells, +1 mapped by
+ * the boundary rule (cells on the high side of an outflow axis are skipped).  Either pointer may be
+ * NULL.  Synchronises. */
+int mhd_diagnostics(mhd_ctx* ctx, double sums[8], double* max_abs_divb);
+
+/* Tuning knobs, all optional: key "segment" = cells per thread along the sweep for the marching
+ * kernels (0 = whole pencil), "block" = threads per block, "path" = 0 auto | 1 generic kernels only.
+ * Unknown keys return MHD_EINVAL. */
+int mhd_set_option(mhd_ctx* ctx, const char* key, long long value);
+
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches claim). */
+long long mhd_launch_count(const mhd_ctx* ctx);
+
+/* Message of the most recent failure on this context ("" if none); valid until the next call on it.
+ * For ctx == NULL returns the message of the last failed mhd_create on this thread. */
+const char* mhd_last_error(const mhd_ctx* ctx);
+
+/* Library version string, e.g. "mhd-b200 0.1 (sm_100a)". */
+const char* mhd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MHD_H_ */

@@ -1,0 +1,445 @@
+// mhd_api.cu -- the C ABI of include/mhd.h: context, SoA device buffers, operator sequencing.
+// PRODUCT code (CUDA path).  No CPU fallback: every step of the hot path runs in the kernels of
+// this directory; if CUDA is unavailable every compute call returns MHD_ECUDA.
+#include "../../include/mhd.h"
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "mhd_generic.cuh"
+
+using namespace mhd;
+
+struct mhd_ctx {
+  int n[3];
+  double gamma;
+  int precision, bc;
+  size_t esize;            // bytes per element
+  size_t N;                // cells
+  size_t field_bytes;      // N*esize rounded up to 256
+  // device memory
+  void* ws;                // workspace base
+  size_t ws_bytes;
+  bool owns_ws;
+  void* cur[8];            // current state, field order rho,mx,my,mz,E,Bx,By,Bz
+  void* alt[8];            // scratch copy (out-of-place operators ping-pong field by field)
+  Scalars* sc;             // device scalar block
+  double* diag;            // device: 8 sums + divb bits
+  cudaStream_t stream;
+  bool owns_stream;
+  bool stream_set;
+  bool has_state;
+  long long step_index;
+  long long launches;
+  // options
+  int opt_segment, opt_block, opt_path;
+  int sm_count;
+  char err[512];
+};
+
+static thread_local char g_create_err[256] = "";
+
+static int fail(mhd_ctx* c, int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  if (c) vsnprintf(c->err, sizeof(c->err), fmt, ap);
+  else vsnprintf(g_create_err, sizeof(g_create_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_TRY(c, expr)                                                                       \
+  do {                                                                                          \
+    cudaError_t e_ = (expr);                                                                    \
+    if (e_ != cudaSuccess) return fail((c), MHD_ECUDA, "%s failed: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+static size_t round256(size_t x) { return (x + 255) & ~(size_t)255; }
+static const size_t kScalarBlock = 1024;   // Scalars + diagnostics scratch
+
+static bool shape_ok(int nx, int ny, int nz, int precision) {
+  if (nx < 1 || ny < 1 || nz < 1) return false;
+  if (precision != MHD_F32 && precision != MHD_F64) return false;
+  if ((double)nx * ny * nz > 4.0e9) return false;
+  return true;
+}
+
+extern "C" size_t mhd_workspace_bytes(int nx, int ny, int nz, int precision) {
+  if (!shape_ok(nx, ny, nz, precision)) return 0;
+  const size_t es = precision == MHD_F32 ? 4 : 8;
+  const size_t fb = round256((size_t)nx * ny * nz * es);
+  return 16 * fb + kScalarBlock;
+}
+
+extern "C" const char* mhd_version(void) { return "mhd-b200 0.1 (sm_100a)"; }
+
+extern "C" const char* mhd_last_error(const mhd_ctx* c) { return c ? c->err : g_create_err; }
+
+extern "C" long long mhd_launch_count(const mhd_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, int bc, mhd_ctx** out) {
+  if (!out) return fail(nullptr, MHD_EINVAL, "mhd_create: out is NULL");
+  *out = nullptr;
+  if (!shape_ok(nx, ny, nz, precision)) return fail(nullptr, MHD_EINVAL, "mhd_create: bad extents or precision");
+  if (!(gamma > 1.0)) return fail(nullptr, MHD_EINVAL, "mhd_create: gamma must be > 1");
+  if (bc != MHD_BC_PERIODIC && bc != MHD_BC_OUTFLOW) return fail(nullptr, MHD_EINVAL, "mhd_create: unknown bc");
+  mhd_ctx* c = new (std::nothrow) mhd_ctx();
+  if (!c) return fail(nullptr, MHD_ENOMEM, "mhd_create: out of host memory");
+  memset(c, 0, sizeof(*c));
+  c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
+  c->gamma = gamma; c->precision = precision; c->bc = bc;
+  c->esize = precision == MHD_F32 ? 4 : 8;
+  c->N = (size_t)nx * ny * nz;
+  c->field_bytes = round256(c->N * c->esize);
+  c->opt_segment = -1;   // auto
+  c->opt_block = 128;
+  c->opt_path = 0;
+  c->sm_count = 148;
+  *out = c;
+  return MHD_OK;
+}
+
+static int carve(mhd_ctx* c) {
+  char* base = (char*)c->ws;
+  for (int f = 0; f < 8; ++f) {
+    c->cur[f] = base + (size_t)f * c->field_bytes;
+    c->alt[f] = base + (size_t)(8 + f) * c->field_bytes;
+  }
+  c->sc = (Scalars*)(base + 16 * c->field_bytes);
+  c->diag = (double*)(base + 16 * c->field_bytes + 256);
+  CUDA_TRY(c, cudaMemsetAsync(c->sc, 0, kScalarBlock, c->stream));
+  return MHD_OK;
+}
+
+static int ensure_ready(mhd_ctx* c) {
+  if (!c->stream_set) {
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking));
+    c->owns_stream = true;
+    c->stream_set = true;
+  }
+  if (!c->ws) {
+    c->ws_bytes = mhd_workspace_bytes(c->n[0], c->n[1], c->n[2], c->precision);
+    cudaError_t e = cudaMalloc(&c->ws, c->ws_bytes);
+    if (e != cudaSuccess) {
+      c->ws = nullptr;
+      return fail(c, e == cudaErrorMemoryAllocation ? MHD_ENOMEM : MHD_ECUDA, "cudaMalloc(%zu) failed: %s", c->ws_bytes,
+                  cudaGetErrorString(e));
+    }
+    c->owns_ws = true;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      c->sm_count = sms;
+    return carve(c);
+  }
+  return MHD_OK;
+}
+
+extern "C" int mhd_bind(mhd_ctx* c, void* device_workspace, size_t bytes, void* cuda_stream) {
+  if (!c) return MHD_EINVAL;
+  if (c->has_state || c->ws) return fail(c, MHD_EINVAL, "mhd_bind: must precede mhd_set_state");
+  c->stream = (cudaStream_t)cuda_stream;
+  c->owns_stream = false;
+  c->stream_set = true;
+  if (device_workspace) {
+    const size_t need = mhd_workspace_bytes(c->n[0], c->n[1], c->n[2], c->precision);
+    if (bytes < need) return fail(c, MHD_ENOMEM, "mhd_bind: workspace of %zu bytes < %zu needed", bytes, need);
+    if (((size_t)device_workspace & 255) != 0) return fail(c, MHD_ENOMEM, "mhd_bind: workspace not 256-byte aligned");
+    c->ws = device_workspace;
+    c->ws_bytes = bytes;
+    c->owns_ws = false;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      c->sm_count = sms;
+    return carve(c);
+  }
+  return MHD_OK;
+}
+
+extern "C" int mhd_destroy(mhd_ctx* c) {
+  if (!c) return MHD_OK;
+  if (c->stream_set) cudaStreamSynchronize(c->stream);
+  if (c->owns_ws && c->ws) cudaFree(c->ws);
+  if (c->owns_stream && c->stream_set) cudaStreamDestroy(c->stream);
+  delete c;
+  return MHD_OK;
+}
+
+extern "C" int mhd_set_state(mhd_ctx* c, const void* const fields[8], int where) {
+  if (!c) return MHD_EINVAL;
+  if (!fields || (where != MHD_HOST && where != MHD_DEVICE)) return fail(c, MHD_EINVAL, "mhd_set_state: bad argument");
+  for (int f = 0; f < 8; ++f)
+    if (!fields[f]) return fail(c, MHD_EINVAL, "mhd_set_state: fields[%d] is NULL", f);
+  int rc = ensure_ready(c);
+  if (rc) return rc;
+  const cudaMemcpyKind kind = where == MHD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  for (int f = 0; f < 8; ++f) CUDA_TRY(c, cudaMemcpyAsync(c->cur[f], fields[f], c->N * c->esize, kind, c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->sc, 0, sizeof(Scalars), c->stream));
+  if (where == MHD_HOST) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  c->has_state = true;
+  return MHD_OK;
+}
+
+static int check_poison(mhd_ctx* c, const Scalars& h) {
+  if (h.nonfinite) return fail(c, MHD_ENONFINITE, "c_max reduction saw a non-finite or non-positive value (c_max = %g)", h.cmax);
+  return MHD_OK;
+}
+
+extern "C" int mhd_get_state(mhd_ctx* c, void* const fields[8], int where) {
+  if (!c) return MHD_EINVAL;
+  if (!fields || (where != MHD_HOST && where != MHD_DEVICE)) return fail(c, MHD_EINVAL, "mhd_get_state: bad argument");
+  for (int f = 0; f < 8; ++f)
+    if (!fields[f]) return fail(c, MHD_EINVAL, "mhd_get_state: fields[%d] is NULL", f);
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_get_state: no state set");
+  const cudaMemcpyKind kind = where == MHD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+  for (int f = 0; f < 8; ++f) CUDA_TRY(c, cudaMemcpyAsync(fields[f], c->cur[f], c->N * c->esize, kind, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return MHD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// operator launches
+// ---------------------------------------------------------------------------------------------
+template <class real>
+static SweepGeom<real> make_geom(const mhd_ctx* c, int d) {
+  const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  const long long stride[3] = {1, c->n[0], (long long)c->n[0] * c->n[1]};
+  SweepGeom<real> g;
+  g.nd = c->n[d]; g.na = c->n[t1]; g.nb = c->n[t2];
+  g.sd = stride[d]; g.sa = stride[t1]; g.sb = stride[t2];
+  g.bc = c->bc;
+  g.gamma = (real)c->gamma;
+  // consecutive threads should walk the transverse axis with the smaller stride (x when d != x)
+  g.a_fast = (g.sa < g.sb || g.nb == 1) && g.na > 1 ? 1 : (g.nb > 1 ? 0 : 1);
+  // segment length: whole pencils when that already fills the machine, else split
+  int seg = c->opt_segment;
+  if (seg < 0) {
+    const long long pencils = (long long)g.na * g.nb;
+    const long long want = (long long)c->sm_count * 2048;      // resident-thread capacity
+    seg = g.nd;
+    while (seg > 32 && pencils * ((g.nd + seg - 1) / seg) < want) seg = (seg + 1) / 2;
+  }
+  if (seg == 0 || seg > g.nd) seg = g.nd;
+  g.seg = seg;
+  g.nseg = (g.nd + seg - 1) / seg;
+  return g;
+}
+
+template <class real>
+static int launch_fluid(mhd_ctx* c, int d) {
+  const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  if (c->n[d] == 1) return MHD_OK;   // both face fluxes of the only cell are identical: exact no-op (R10)
+  FluidArgs<real> A;
+  const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
+  for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
+  A.bd = (const real*)c->cur[5 + d]; A.bt1 = (const real*)c->cur[5 + t1]; A.bt2 = (const real*)c->cur[5 + t2];
+  A.dt = &c->sc->dt;
+  A.g = make_geom<real>(c, d);
+  const long long threads = (long long)A.g.na * A.g.nb * A.g.nseg;
+  const int block = c->opt_block;
+  const unsigned grid = (unsigned)((threads + block - 1) / block);
+  fluid_march_kernel<real><<<grid, block, 0, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  for (int k = 0; k < 5; ++k) { void* t = c->cur[role[k]]; c->cur[role[k]] = c->alt[role[k]]; c->alt[role[k]] = t; }
+  return MHD_OK;
+}
+
+template <class real>
+static int launch_bpair(mhd_ctx* c, int d, int t2_first) {
+  const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  BPairArgs<real> A;
+  A.rho = (const real*)c->cur[0]; A.md = (const real*)c->cur[1 + d];
+  A.bd = (const real*)c->cur[5 + d]; A.bt1 = (const real*)c->cur[5 + t1]; A.bt2 = (const real*)c->cur[5 + t2];
+  A.bdo = (real*)c->alt[5 + d]; A.bt1o = (real*)c->alt[5 + t1]; A.bt2o = (real*)c->alt[5 + t2];
+  A.dt = &c->sc->dt;
+  A.t2_first = t2_first;
+  A.g = make_geom<real>(c, d);
+  const long long threads = (long long)A.g.na * A.g.nb * A.g.nseg;
+  const int block = c->opt_block;
+  const unsigned grid = (unsigned)((threads + block - 1) / block);
+  bpair_march_kernel<real><<<grid, block, 0, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  return MHD_OK;
+}
+
+template <class real>
+static int launch_cfl(mhd_ctx* c) {
+  CflArgs<real> A;
+  for (int f = 0; f < 8; ++f) A.f[f] = (const real*)c->cur[f];
+  A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2]; A.bc = c->bc;
+  A.gamma = (real)c->gamma;
+  A.cmax_bits = &c->sc->cmax_bits;
+  const int block = 256;
+  long long want = ((long long)c->N + block - 1) / block;
+  const long long cap = (long long)c->sm_count * 8;
+  const unsigned grid = (unsigned)(want < cap ? want : cap);
+  cfl_kernel<real><<<grid, block, 0, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return MHD_OK;
+}
+
+#define BY_PRECISION(c, CALL32, CALL64) ((c)->precision == MHD_F32 ? (CALL32) : (CALL64))
+
+static int sweep(mhd_ctx* c, int d, bool reverse) {
+  int rc;
+  if (!reverse) {
+    if ((rc = BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d)))) return rc;
+    return BY_PRECISION(c, launch_bpair<float>(c, d, 0), launch_bpair<double>(c, d, 0));
+  }
+  if ((rc = BY_PRECISION(c, launch_bpair<float>(c, d, 1), launch_bpair<double>(c, d, 1)))) return rc;
+  return BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d));
+}
+
+// one double sweep, eqs (23)-(25) PAPER.md:164-170
+static int double_sweep(mhd_ctx* c) {
+  static const int order[3][3] = {{0, 1, 2}, {2, 0, 1}, {1, 2, 0}};
+  const int* o = order[((c->step_index % 3) + 3) % 3];
+  int rc;
+  for (int i = 0; i < 3; ++i) if ((rc = sweep(c, o[i], false))) return rc;
+  for (int i = 2; i >= 0; --i) if ((rc = sweep(c, o[i], true))) return rc;
+  c->step_index++;
+  return MHD_OK;
+}
+
+static int read_scalars(mhd_ctx* c, Scalars* h) {
+  CUDA_TRY(c, cudaMemcpyAsync(h, c->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return MHD_OK;
+}
+
+extern "C" int mhd_cfl_dt(mhd_ctx* c, double cfl, double* dt_out, double* cmax_out) {
+  if (!c) return MHD_EINVAL;
+  if (!(cfl > 0.0) || !dt_out) return fail(c, MHD_EINVAL, "mhd_cfl_dt: bad argument");
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_cfl_dt: no state set");
+  int rc = BY_PRECISION(c, launch_cfl<float>(c), launch_cfl<double>(c));
+  if (rc) return rc;
+  dt_from_cmax_kernel<<<1, 1, 0, c->stream>>>(c->sc, cfl, 0);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  Scalars h;
+  if ((rc = read_scalars(c, &h))) return rc;
+  *dt_out = h.dt;
+  if (cmax_out) *cmax_out = h.cmax;
+  return check_poison(c, h);
+}
+
+extern "C" int mhd_step(mhd_ctx* c, int n, double cfl, double* t_advanced) {
+  if (!c) return MHD_EINVAL;
+  if (n < 0 || !(cfl > 0.0)) return fail(c, MHD_EINVAL, "mhd_step: bad argument");
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_step: no state set");
+  int rc;
+  reset_call_kernel<<<1, 1, 0, c->stream>>>(c->sc);
+  c->launches++;
+  for (int it = 0; it < n; ++it) {
+    if ((rc = BY_PRECISION(c, launch_cfl<float>(c), launch_cfl<double>(c)))) return rc;
+    dt_from_cmax_kernel<<<1, 1, 0, c->stream>>>(c->sc, cfl, 1);
+    c->launches++;
+    if ((rc = double_sweep(c))) return rc;
+  }
+  CUDA_TRY(c, cudaGetLastError());
+  if (t_advanced) {
+    Scalars h;
+    if ((rc = read_scalars(c, &h))) return rc;
+    *t_advanced = h.t_call;
+    return check_poison(c, h);
+  }
+  return MHD_OK;
+}
+
+extern "C" int mhd_step_fixed(mhd_ctx* c, int n, double dt) {
+  if (!c) return MHD_EINVAL;
+  if (n < 0 || !(dt > 0.0)) return fail(c, MHD_EINVAL, "mhd_step_fixed: bad argument");
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_step_fixed: no state set");
+  set_dt_kernel<<<1, 1, 0, c->stream>>>(c->sc, dt, n);
+  c->launches++;
+  int rc;
+  for (int it = 0; it < n; ++it)
+    if ((rc = double_sweep(c))) return rc;
+  CUDA_TRY(c, cudaGetLastError());
+  return MHD_OK;
+}
+
+extern "C" int mhd_apply(mhd_ctx* c, int op, int d, int reverse, double dt) {
+  if (!c) return MHD_EINVAL;
+  if (d < 0 || d > 2 || !(dt > 0.0)) return fail(c, MHD_EINVAL, "mhd_apply: bad argument");
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_apply: no state set");
+  set_dt_kernel<<<1, 1, 0, c->stream>>>(c->sc, dt, 0);
+  c->launches++;
+  switch (op) {
+    case MHD_OP_FLUID: return BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d));
+    case MHD_OP_BPAIR:
+      return BY_PRECISION(c, launch_bpair<float>(c, d, reverse ? 1 : 0), launch_bpair<double>(c, d, reverse ? 1 : 0));
+    case MHD_OP_SWEEP_FORWARD: return sweep(c, d, false);
+    case MHD_OP_SWEEP_REVERSE: return sweep(c, d, true);
+    default: return fail(c, MHD_EINVAL, "mhd_apply: unknown operator %d", op);
+  }
+}
+
+extern "C" int mhd_get_step_index(mhd_ctx* c, long long* s) {
+  if (!c || !s) return MHD_EINVAL;
+  *s = c->step_index;
+  return MHD_OK;
+}
+
+extern "C" int mhd_set_step_index(mhd_ctx* c, long long s) {
+  if (!c) return MHD_EINVAL;
+  c->step_index = s;
+  return MHD_OK;
+}
+
+extern "C" int mhd_get_time(mhd_ctx* c, double* t) {
+  if (!c || !t) return MHD_EINVAL;
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_get_time: no state set");
+  Scalars h;
+  int rc = read_scalars(c, &h);
+  if (rc) return rc;
+  *t = h.t_total;
+  return MHD_OK;
+}
+
+extern "C" int mhd_diagnostics(mhd_ctx* c, double sums[8], double* max_abs_divb) {
+  if (!c) return MHD_EINVAL;
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_diagnostics: no state set");
+  CUDA_TRY(c, cudaMemsetAsync(c->diag, 0, 9 * sizeof(double), c->stream));
+  const int block = 256;
+  long long want = ((long long)c->N + block - 1) / block;
+  const long long cap = (long long)c->sm_count * 8;
+  const unsigned grid = (unsigned)(want < cap ? want : cap);
+  if (c->precision == MHD_F32) {
+    CflArgs<float> A;
+    for (int f = 0; f < 8; ++f) A.f[f] = (const float*)c->cur[f];
+    A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2]; A.bc = c->bc; A.gamma = (float)c->gamma; A.cmax_bits = nullptr;
+    diag_kernel<float><<<grid, block, 0, c->stream>>>(A, c->diag, (unsigned long long*)(c->diag + 8));
+  } else {
+    CflArgs<double> A;
+    for (int f = 0; f < 8; ++f) A.f[f] = (const double*)c->cur[f];
+    A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2]; A.bc = c->bc; A.gamma = c->gamma; A.cmax_bits = nullptr;
+    diag_kernel<double><<<grid, block, 0, c->stream>>>(A, c->diag, (unsigned long long*)(c->diag + 8));
+  }
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  double h[9];
+  CUDA_TRY(c, cudaMemcpyAsync(h, c->diag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (sums) memcpy(sums, h, 8 * sizeof(double));
+  if (max_abs_divb) *max_abs_divb = h[8];   // the bit pattern of a non-negative double IS that double
+  return MHD_OK;
+}
+
+extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
+  if (!c || !key) return MHD_EINVAL;
+  if (!strcmp(key, "segment")) { if (value < -1) return fail(c, MHD_EINVAL, "segment < -1"); c->opt_segment = (int)value; return MHD_OK; }
+  if (!strcmp(key, "block")) {
+    if (value < 32 || value > 256 || (value & 31)) return fail(c, MHD_EINVAL, "block must be a multiple of 32 in [32,256]");
+    c->opt_block = (int)value; return MHD_OK;
+  }
+  if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
+  return fail(c, MHD_EINVAL, "unknown option '%s'", key);
+}

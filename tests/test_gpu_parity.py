@@ -1,0 +1,285 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element  (-m gpu).
+
+Tolerances (BASELINE.json north_star):
+  fp64: 1e-12 max relative error per step (per field group: max|gpu-oracle| / max|oracle|)
+  fp32: 1e-5 after one step, against oracle<double> run from the fp32-rounded inputs with the same dt;
+        1e-3 L1 after 100 steps.
+"""
+import ctypes
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_0908_4362_b200 import inputs
+from tests.parity_utils import l1_rel, max_rel, random_state, worst
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32_STEP = 1e-5
+TOL32_L1_100 = 1e-3
+
+P, O = inputs.PERIODIC, inputs.OUTFLOW
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_0908_4362_b200 import binding
+    return binding
+
+
+def _solver(B, f, gamma, bc, prec, **opts):
+    nz, ny, nx = f[0].shape
+    s = B.Solver(nx, ny, nz, gamma, prec, bc)
+    for k, v in opts.items():
+        s.set_option(k, v)
+    dt = np.float32 if prec == "f32" else np.float64
+    s.set_state([np.ascontiguousarray(a, dtype=dt) for a in f])
+    return s
+
+
+def _ref_input(f, prec):
+    """oracle<double> input: the run-precision-rounded state, widened back to float64"""
+    dt = np.float32 if prec == "f32" else np.float64
+    return [np.array(np.asarray(a, dtype=dt), dtype=np.float64) for a in f]
+
+
+SHAPES = [(40, 24, 20), (48, 1, 1), (1, 40, 1), (1, 1, 36), (32, 20, 1), (1, 24, 16), (20, 1, 24), (7, 5, 3)]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("bc", [P, O])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_each_operator_matches_oracle(B, shape, bc, prec):
+    nx, ny, nz = shape
+    f0 = random_state(nx, ny, nz, seed=nx * 7 + ny * 3 + nz + bc)
+    gamma, dt = 5.0 / 3.0, 0.21
+    tol = TOL64 if prec == "f64" else TOL32_STEP
+    for d in range(3):
+        for op, rev in [(B.MHD_OP_FLUID, 0), (B.MHD_OP_BPAIR, 0), (B.MHD_OP_BPAIR, 1),
+                        (B.MHD_OP_SWEEP_FORWARD, 0), (B.MHD_OP_SWEEP_REVERSE, 0)]:
+            ref = _ref_input(f0, prec)
+            t1, t2 = (d + 1) % 3, (d + 2) % 3
+            if op == B.MHD_OP_FLUID:
+                oracle.fluid(ref, gamma, bc, d, dt)
+            elif op == B.MHD_OP_BPAIR:
+                for t in ((t2, t1) if rev else (t1, t2)):
+                    oracle.badvect(ref, gamma, bc, d, t, dt)
+            else:
+                oracle.sweep(ref, gamma, bc, d, op == B.MHD_OP_SWEEP_REVERSE, dt)
+            s = _solver(B, f0, gamma, bc, prec)
+            s.apply(op, d, rev, dt)
+            got = s.get_state()
+            s.close()
+            e = max_rel(got, ref)
+            assert worst(e) <= tol, (shape, bc, prec, d, op, rev, e)
+
+
+@pytest.mark.parametrize("seg", [0, 5, 13, 64])
+@pytest.mark.parametrize("block", [32, 96, 256])
+def test_segment_and_block_options_do_not_change_results(B, seg, block):
+    """ragged tails: segment lengths that do not divide the extent, blocks that do not divide the pencil count"""
+    f0 = random_state(37, 21, 11, seed=5)
+    gamma, dt = 1.4, 0.17
+    ref = _ref_input(f0, "f64")
+    for s_idx in range(3):
+        oracle.step_fixed(ref, gamma, P, s_idx, dt)
+    s = _solver(B, f0, gamma, P, "f64", segment=seg, block=block)
+    s.step_fixed(3, dt)
+    got = s.get_state()
+    assert s.step_index == 3
+    s.close()
+    assert worst(max_rel(got, ref)) <= 3 * TOL64
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("bc", [P, O])
+def test_three_steps_all_rotations(B, prec, bc):
+    f0 = random_state(48, 32, 24, seed=11)
+    gamma, dt = 5.0 / 3.0, 0.15
+    tol = TOL64 if prec == "f64" else TOL32_STEP
+    for s0 in range(3):            # each rotation as a single step from the same state
+        ref = _ref_input(f0, prec)
+        oracle.step_fixed(ref, gamma, bc, s0, dt)
+        s = _solver(B, f0, gamma, bc, prec)
+        s.step_index = s0
+        s.step_fixed(1, dt)
+        got = s.get_state()
+        s.close()
+        e = max_rel(got, ref)
+        assert worst(e) <= tol, (prec, bc, s0, e)
+
+
+def test_cfl_dt_matches_oracle(B):
+    for prec in ("f64", "f32"):
+        for bc in (P, O):
+            f0 = random_state(33, 17, 9, seed=3)
+            ref = _ref_input(f0, prec)
+            cm = oracle.cmax(ref, 5.0 / 3.0, bc)
+            s = _solver(B, f0, 5.0 / 3.0, bc, prec)
+            dt, cmg = s.cfl_dt(0.8)
+            s.close()
+            tol = 1e-14 if prec == "f64" else 2e-6
+            assert abs(cmg - cm) <= tol * cm
+            assert abs(dt - 0.8 / cmg) <= 1e-15 * dt
+
+
+def test_step_with_cfl_matches_oracle_run_fp64(B):
+    f, meta = inputs.orszag_tang(64)
+    ref = _ref_input(f, "f64")
+    t_ref = oracle.run(ref, meta["gamma"], meta["bc"], 0, 12, 0.8)
+    s = _solver(B, f, meta["gamma"], meta["bc"], "f64")
+    t = s.step(12, 0.8)
+    got = s.get_state()
+    assert abs(s.time() - t) < 1e-15 * t
+    s.close()
+    assert abs(t - t_ref) <= 1e-12 * t_ref
+    assert worst(max_rel(got, ref)) <= 12 * TOL64
+
+
+def test_config1_brio_wu_full_run_fp64(B):
+    """BASELINE.json configs[0]: 512x1x1, outflow, cfl 0.8 to t = 0.1, last step clipped (reading R14)"""
+    f, meta = inputs.brio_wu(512)
+    ref = _ref_input(f, "f64")
+    s = _solver(B, f, meta["gamma"], meta["bc"], "f64")
+    t_end, t, k = 0.1 * 512, 0.0, 0
+    worst_step = 0.0
+    while t < t_end - 1e-12:
+        dt_gpu, _ = s.cfl_dt(0.8)
+        dt = min(dt_gpu, 0.5 * (t_end - t))
+        # per-step parity: both sides advance one step from the SAME state with the SAME dt
+        cur = s.get_state()
+        refstep = [a.copy() for a in cur]
+        oracle.step_fixed(refstep, meta["gamma"], meta["bc"], k, dt)
+        oracle.step_fixed(ref, meta["gamma"], meta["bc"], k, dt)
+        s.step_fixed(1, dt)
+        worst_step = max(worst_step, worst(max_rel(s.get_state(), refstep)))
+        t += 2 * dt
+        k += 1
+    got = s.get_state()
+    s.close()
+    assert 100 < k < 200
+    assert worst_step <= TOL64, worst_step
+    assert worst(max_rel(got, ref)) <= 1e-10            # accumulated over ~143 steps
+    assert np.all(got[5] == 0.75) and not got[3].any() and not got[7].any()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config2_orszag_tang_256(B, prec):
+    """BASELINE.json configs[1]: 256x256x1 periodic; per-step parity for s = 0,1,2 at full size, then drift"""
+    f, meta = inputs.orszag_tang(256)
+    gamma, bc = meta["gamma"], meta["bc"]
+    s = _solver(B, f, gamma, bc, prec)
+    tol = TOL64 if prec == "f64" else TOL32_STEP
+    for k in range(3):
+        dt, _ = s.cfl_dt(0.8)
+        cur = s.get_state()
+        ref = [np.array(a, dtype=np.float64) for a in cur]
+        oracle.step_fixed(ref, gamma, bc, k, dt)
+        s.step_fixed(1, dt)
+        e = max_rel(s.get_state(), ref)
+        assert worst(e) <= tol, (k, e)
+    s.close()
+    # multi-step drift: 100 steps with the oracle's own dt sequence (fp32: L1 <= 1e-3)
+    ref = _ref_input(f, prec)
+    s = _solver(B, f, gamma, bc, prec)
+    for k in range(100):
+        dt = 0.8 / oracle.cmax(ref, gamma, bc)
+        oracle.step_fixed(ref, gamma, bc, k, dt)
+        s.step_fixed(1, dt)
+    got = s.get_state()
+    sums, dv = s.diagnostics()
+    s.close()
+    e = l1_rel(got, ref)
+    assert worst(e) <= (TOL32_L1_100 if prec == "f32" else 1e-9), e
+    if prec == "f64":
+        assert dv <= 1e-12 * max(np.abs(got[5]).max(), np.abs(got[6]).max())
+
+
+def test_fp32_l1_after_100_steps_3d(B):
+    f, meta = inputs.turbulence(48, 48, 48)
+    gamma, bc = meta["gamma"], meta["bc"]
+    ref = _ref_input(f, "f32")
+    s = _solver(B, f, gamma, bc, "f32")
+    for k in range(100):
+        dt = 0.8 / oracle.cmax(ref, gamma, bc)
+        oracle.step_fixed(ref, gamma, bc, k, dt)
+        s.step_fixed(1, dt)
+    got = s.get_state()
+    s.close()
+    e = l1_rel(got, ref)
+    assert worst(e) <= TOL32_L1_100, e
+
+
+def test_conservation_and_divb_on_gpu_fp64(B):
+    f, meta = inputs.turbulence(32, 32, 32)
+    s = _solver(B, f, meta["gamma"], meta["bc"], "f64")
+    sums0, dv0 = s.diagnostics()
+    s.step(10, 0.8)
+    sums1, dv1 = s.diagnostics()
+    got = s.get_state()
+    s.close()
+    for i, (a, b) in enumerate(zip(sums0, sums1)):
+        scale = float(np.abs(f[i]).sum())
+        assert abs(a - b) <= 1e-12 * scale, (i, a, b)
+    assert dv1 <= 1e-12 * max(np.abs(g).max() for g in got[5:])
+    # diagnostics agree with numpy
+    for i in range(8):
+        assert abs(sums1[i] - float(got[i].sum())) <= 1e-10 * float(np.abs(got[i]).sum())
+
+
+def test_nonfinite_state_is_reported(B):
+    f, meta = inputs.turbulence(16, 16, 16)
+    f = [a.copy() for a in f]
+    f[0][3, 4, 5] = np.nan
+    s = _solver(B, f, meta["gamma"], meta["bc"], "f64")
+    with pytest.raises(B.MHDError) as ei:
+        s.cfl_dt(0.8)
+    assert ei.value.code == B.MHD_ENONFINITE
+    with pytest.raises(B.MHDError) as ei:
+        s.step(1, 0.8)
+    assert ei.value.code == B.MHD_ENONFINITE
+    s.close()
+
+
+def test_bind_torch_workspace_and_stream_device_state(B):
+    import torch
+    f, meta = inputs.turbulence(24, 16, 8)
+    nz, ny, nx = f[0].shape
+    nbytes = B.mhd_workspace_bytes(nx, ny, nz, B.MHD_F64)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.Stream()
+    s = B.Solver(nx, ny, nz, meta["gamma"], "f64", meta["bc"], workspace=ws, stream=stream)
+    dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in f]
+    torch.cuda.synchronize()
+    s.set_state(dev)
+    s.step_fixed(2, 0.1)
+    out = [torch.empty_like(a) for a in dev]
+    s.get_state(out)
+    ref = _ref_input(f, "f64")
+    oracle.step_fixed(ref, meta["gamma"], meta["bc"], 0, 0.1)
+    oracle.step_fixed(ref, meta["gamma"], meta["bc"], 1, 0.1)
+    assert worst(max_rel([o.cpu().numpy() for o in out], ref)) <= 2 * TOL64
+    assert s.launch_count() > 0
+    s.close()
+    # too-small workspace is refused
+    with pytest.raises(B.MHDError) as ei:
+        B.Solver(nx, ny, nz, meta["gamma"], "f64", meta["bc"], workspace=ws[: nbytes // 2])
+    assert ei.value.code == B.MHD_ENOMEM
+
+
+def test_uniform_state_fixed_point_and_empty_step_count(B):
+    shape = (6, 5, 4)
+    vals = [1.3, 0.4, -0.7, 0.2, 3.1, 0.6, -0.3, 0.9]
+    f = [np.full(shape, v) for v in vals]
+    s = _solver(B, f, 5.0 / 3.0, P, "f64")
+    s.step_fixed(0, 0.3)            # n = 0 is allowed and does nothing
+    s.step_fixed(3, 0.3)
+    got = s.get_state()
+    s.close()
+    for a, b in zip(f, got):
+        assert np.array_equal(a, b)
