@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s of the MHD step on B200 (one JSON line; contract in DESIGN.md "Measurement").
+
+A "step" is one pass of the whole hot path over the resident state: one c_max reduction, dt = cfl/c_max on
+the device, six L_i operators (fluid + B pair each), t += 2 dt.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3|small] [--impl reference]
+
+N > 1: one process per GPU under torchrun, each rank advances its own replica of the workload ("replicas
+only": the paper's method is single-GPU); value = cells advanced by all ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+WORKLOADS = {
+    # name: (generator, n, precision, BASELINE.json config)
+    "c4": ("turbulence", 512, "f32", "configs[3]: 3-D turbulence-like state, 512^3, fp32, periodic, cfl 0.8"),
+    "c5": ("turbulence", 512, "f64", "configs[4]: same seeded state, 512^3, fp64, periodic, cfl 0.8"),
+    "c3": ("blast3d", 256, "f32", "configs[2]: 3-D MHD blast wave, 256^3, fp32, periodic, cfl 0.8"),
+    "small": ("turbulence", 128, "f32", "reduced 128^3 fp32 turbulence-like state (not a BASELINE config)"),
+}
+ALGO_WORDS_STEP = 96          # ideal: each of the six L_i reads 8 fields and writes 8
+CFL = 0.8
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.06] or [r for (_, r) in self.rows[-3:]]
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            c = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(c[0])); smax.append(float(c[1])); pw.append(float(c[2]))
+            except Exception:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_state(gen, n, prec, device):
+    """seeded synthetic state of the workload, built on the device with torch (plumbing), in run precision"""
+    import torch
+    from paper_0908_4362_b200 import inputs
+    kw = dict(xp=torch, xp_kw={"device": device})
+    f, meta = (inputs.turbulence(n, **kw) if gen == "turbulence" else inputs.blast3d(n, **kw))
+    dt = torch.float32 if prec == "f32" else torch.float64
+    out = [a.to(dt).contiguous() for a in f]
+    del f
+    torch.cuda.empty_cache()
+    return out, meta
+
+
+def oracle_rate(gen, prec, budget_s=12.0, n=96):
+    """the oracle as it stands, timed on the host cores on a bounded sample of the workload"""
+    import oracle
+    from paper_0908_4362_b200 import inputs
+    f, meta = (inputs.turbulence(n) if gen == "turbulence" else inputs.blast3d(n))
+    dt = np.float32 if prec == "f32" else np.float64
+    st = [np.array(a, dtype=dt) for a in f]
+    oracle.run(st, meta["gamma"], meta["bc"], 0, 1, CFL)            # page in / warm caches
+    steps, t0 = 0, time.perf_counter()
+    while True:
+        oracle.run(st, meta["gamma"], meta["bc"], steps + 1, 1, CFL)
+        steps += 1
+        el = time.perf_counter() - t0
+        if el > budget_s or steps >= 200:
+            break
+    return (n ** 3) * steps / el, oracle.num_threads(), f"{gen} {n}^3 {prec}, {steps} steps in {el:.1f} s"
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle (deliberately slow CPU program), same metric/config keys"""
+    if rank != 0:
+        return
+    gen, n, prec, desc = WORKLOADS[args.workload]
+    import oracle
+    from paper_0908_4362_b200 import inputs
+    ns = 96 if n >= 96 else n
+    f, meta = (inputs.turbulence(ns) if gen == "turbulence" else inputs.blast3d(ns))
+    dt = np.float32 if prec == "f32" else np.float64
+    st = [np.array(a, dtype=dt) for a in f]
+    k0 = 0
+    for _ in range(args.warmup):
+        oracle.run(st, meta["gamma"], meta["bc"], k0, 1, CFL); k0 += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.run(st, meta["gamma"], meta["bc"], k0, 1, CFL); k0 += 1
+    el = time.perf_counter() - t0
+    val = ns ** 3 * args.steps / el
+    sample = f"{gen} {ns}^3 {prec} sub-sample of the {n}^3 workload, {args.steps} steps"
+    print(json.dumps({
+        "impl": "reference", "metric": "MHD cell-updates/sec", "value": val, "unit": "cell-updates/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {desc}", "cfl": CFL, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "cell-updates/s", "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-breakdown", action="store_true")
+    ap.add_argument("--option", action="append", default=[], help="key=value passed to mhd_set_option")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_0908_4362_b200 import binding as B      # raises if libmhd.so is missing: no fallback
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    device = f"cuda:{local_rank}"
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    gen, n, prec, desc = WORKLOADS[args.workload]
+    N = n ** 3
+    esize = 4 if prec == "f32" else 8
+    state, meta = make_state(gen, n, prec, device)
+    ws = torch.empty(B.mhd_workspace_bytes(n, n, n, B.MHD_F32 if prec == "f32" else B.MHD_F64), dtype=torch.uint8, device=device)
+    stream = torch.cuda.Stream(device=device)
+    sol = B.Solver(n, n, n, meta["gamma"], prec, meta["bc"], workspace=ws, stream=stream)
+    for kv in args.option:
+        k, v = kv.split("=")
+        sol.set_option(k, int(v))
+    torch.cuda.synchronize()
+    sol.set_state(state)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    # ---- device-resident throughput -----------------------------------------------------------
+    with torch.cuda.stream(stream):
+        sol.step(args.warmup, CFL, sync=True)
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        time.sleep(0.15)
+        barrier()
+        l0 = sol.launch_count()
+        e0, e1 = ev(), ev()
+        w0 = time.time()
+        e0.record(stream)
+        sol.step(args.steps, CFL, sync=False)
+        e1.record(stream)
+        barrier()
+        w1 = time.time()
+        l1 = sol.launch_count()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(w0, w1)
+    if world > 1:
+        t = torch.tensor([ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    t_now = sol.time()        # also surfaces a poisoned state
+    value = N * world * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel breakdown and roofline of the dominant kernel (rank 0) ---------------------
+    peak, peak_src = peaks()
+    roofline, breakdown = None, None
+    if rank == 0 and not args.no_breakdown:
+        dtv, _ = sol.cfl_dt(CFL)
+        kinds = [("fluid_x", B.MHD_OP_FLUID, 0, 13), ("fluid_y", B.MHD_OP_FLUID, 1, 13), ("fluid_z", B.MHD_OP_FLUID, 2, 13),
+                 ("bpair_x", B.MHD_OP_BPAIR, 0, 8), ("bpair_y", B.MHD_OP_BPAIR, 1, 8), ("bpair_z", B.MHD_OP_BPAIR, 2, 8)]
+        breakdown = {}
+        reps = 5
+        with torch.cuda.stream(stream):
+            for name, op, d, words in kinds:
+                sol.apply(op, d, 0, dtv)                       # warm
+                a, b = ev(), ev()
+                torch.cuda.synchronize()
+                a.record(stream)
+                for _ in range(reps):
+                    sol.apply(op, d, 0, dtv)
+                b.record(stream)
+                torch.cuda.synchronize()
+                kms = a.elapsed_time(b) / reps                 # includes the 1-thread set_dt launch (~2 us)
+                breakdown[name] = {"ms": kms, "algo_GBps": words * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": words}
+            a, b = ev(), ev()
+            torch.cuda.synchronize()
+            a.record(stream)
+            for _ in range(reps):
+                sol.cfl_dt(CFL)
+            b.record(stream)
+            torch.cuda.synchronize()
+            kms = a.elapsed_time(b) / reps
+            breakdown["cfl"] = {"ms": kms, "algo_GBps": 8 * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": 8}
+        # dominant kernel = the fluid kernel with the largest share of a step (each runs twice per step)
+        dom = max(("fluid_x", "fluid_y", "fluid_z"), key=lambda k: breakdown[k]["ms"])
+        ach = breakdown[dom]["algo_GBps"]
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": None, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": 13 * esize * N,
+                    "step": {"algorithmic_bytes_per_cell_step": ALGO_WORDS_STEP * esize,
+                             "achieved": ALGO_WORDS_STEP * esize * (value / world) / 1e9,
+                             "frac": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / peak}}
+
+    # ---- end to end through the C ABI with HOST buffers ----------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        host = [torch.empty((n, n, n), dtype=state[0].dtype, pin_memory=True) for _ in range(8)]
+        for h, s in zip(host, state):
+            h.copy_(s)
+        torch.cuda.synchronize()
+        k_e2e = 2
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            sol.set_state(host)                    # H2D of the step's inputs (pinned host memory)
+            sol.step(1, CFL, sync=True)
+            sol.get_state(host)                    # D2H of the step's result
+        barrier()
+        el = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([el], device=device, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        e2e = {"value": N * world * k_e2e / el, "unit": "cell-updates/s", "h2d_bytes_per_step": 8 * N * esize,
+               "d2h_bytes_per_step": 8 * N * esize, "steps": k_e2e}
+        del host
+
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        v, cores, sample = oracle_rate(gen, prec)
+        cpu = {"value": v, "unit": "cell-updates/s", "cores": cores, "kind": "oracle", "sample": sample}
+
+    if rank == 0:
+        out = {
+            "metric": "MHD cell-updates/sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
+            "config": {"workload": f"{args.workload}: {desc}", "grid": [n, n, n], "cfl": CFL, "gamma": meta["gamma"],
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": f"state {8 * N * esize / 1e9:.2f} GB per copy >> 126 MB L2 (inputs larger than L2, no flush needed)",
+                       "t_grid_after": t_now},
+            "clocks": clocks, "gpu_launches": int(l1 - l0), "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+            "kernels": breakdown,
+        }
+        print(json.dumps(out))
+    sol.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
