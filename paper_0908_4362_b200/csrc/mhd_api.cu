@@ -9,6 +9,8 @@
 #include <new>
 
 #include "mhd_generic.cuh"
+#include "mhd_yz.cuh"
+#include "mhd_x.cuh"
 
 using namespace mhd;
 
@@ -228,10 +230,143 @@ static SweepGeom<real> make_geom(const mhd_ctx* c, int d) {
   return g;
 }
 
+// ---- fast path for sweeps along y and z (mhd_yz.cuh) ----------------------------------------
+static const int kYZBlock = 128;
+
+static bool yz_ok(const mhd_ctx* c, int d) {
+  return c->opt_path == 0 && d != 0 && c->n[d] >= 8 && c->n[0] >= 32 && c->N < ((size_t)1 << 31);
+}
+
+template <class real>
+static YZArgs<real> make_yz(mhd_ctx* c, int d) {
+  const int o = 3 - d;                        // the other transverse axis (x is always one of them)
+  const int stride[3] = {1, c->n[0], c->n[0] * c->n[1]};
+  YZArgs<real> A;
+  memset(&A, 0, sizeof(A));
+  A.nx = c->n[0]; A.nd = c->n[d]; A.no = c->n[o];
+  A.sd = stride[d]; A.so = stride[o];
+  A.bc = c->bc;
+  A.x_is_t1 = (d == 2) ? 1 : 0;               // z: (t1,t2) = (x,y);  y: (t1,t2) = (z,x)
+  A.gamma = (real)c->gamma;
+  A.dt = &c->sc->dt;
+  int seg = c->opt_segment;
+  if (seg < 0) {
+    const long long pencils = (long long)A.nx * A.no;
+    const long long want = (long long)c->sm_count * 1024;
+    seg = A.nd;
+    while (seg > 64 && pencils * ((A.nd + seg - 1) / seg) < want) seg = (seg + 1) / 2;
+  }
+  if (seg == 0 || seg > A.nd) seg = A.nd;
+  A.seg = seg;
+  return A;
+}
+
+template <class real>
+static dim3 yz_grid(const YZArgs<real>& A) {
+  return dim3((A.nx + kYZBlock - 1) / kYZBlock, A.no, (A.nd + A.seg - 1) / A.seg);
+}
+
+template <class real>
+static int launch_fluid_yz(mhd_ctx* c, int d) {
+  const int t1 = (d + 1) % 3, t2 = (d + 2) % 3, o = 3 - d;
+  YZArgs<real> A = make_yz<real>(c, d);
+  const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
+  for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
+  A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
+  fluid_yz_kernel<real, kYZBlock><<<yz_grid(A), kYZBlock, 0, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  for (int k = 0; k < 5; ++k) { void* t = c->cur[role[k]]; c->cur[role[k]] = c->alt[role[k]]; c->alt[role[k]] = t; }
+  return MHD_OK;
+}
+
+template <class real>
+static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
+  const int o = 3 - d;
+  YZArgs<real> A = make_yz<real>(c, d);
+  A.u[0] = (const real*)c->cur[0]; A.u[1] = (const real*)c->cur[1 + d];
+  A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
+  A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];
+  A.t2_first = t2_first;
+  bpair_yz_kernel<real, kYZBlock><<<yz_grid(A), kYZBlock, 0, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  return MHD_OK;
+}
+
+// ---- fast path for sweeps along x (mhd_x.cuh) -------------------------------------------------
+template <class real>
+static bool x_ok(const mhd_ctx* c) {
+  const int V = VecOf<real>::V;
+  return c->opt_path == 0 && c->bc == MHD_BC_PERIODIC && c->n[0] % V == 0 && c->n[0] / V <= 256 &&
+         c->N < ((size_t)1 << 31);
+}
+
+template <class real>
+static XArgs<real> make_x(mhd_ctx* c, int* block, unsigned* grid) {
+  const int V = VecOf<real>::V;
+  XArgs<real> A;
+  memset(&A, 0, sizeof(A));
+  A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2];
+  A.tpr = A.nx / V;
+  A.rpb = A.tpr >= 128 ? 1 : 128 / A.tpr;
+  const int nrows = A.ny * A.nz;
+  if (A.rpb > nrows) A.rpb = nrows;
+  A.gamma = (real)c->gamma;
+  A.dt = &c->sc->dt;
+  *block = A.tpr * A.rpb;
+  *grid = (unsigned)((nrows + A.rpb - 1) / A.rpb);
+  return A;
+}
+
+template <class real>
+static int launch_fluid_x(mhd_ctx* c) {
+  int block; unsigned grid;
+  XArgs<real> A = make_x<real>(c, &block, &grid);
+  const int role[5] = {0, 1, 2, 3, 4};
+  for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
+  A.bx = (const real*)c->cur[5]; A.by = (const real*)c->cur[6]; A.bz = (const real*)c->cur[7];
+  const size_t smem = (size_t)35 * block * sizeof(real);
+  static bool attr_set = false;
+  if (!attr_set) {
+    CUDA_TRY(c, cudaFuncSetAttribute(fluid_x_kernel<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, 35 * 256 * (int)sizeof(real)));
+    attr_set = true;
+  }
+  fluid_x_kernel<real><<<grid, block, smem, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  for (int k = 0; k < 5; ++k) { void* t = c->cur[role[k]]; c->cur[role[k]] = c->alt[role[k]]; c->alt[role[k]] = t; }
+  return MHD_OK;
+}
+
+template <class real>
+static int launch_bpair_x(mhd_ctx* c, int t2_first) {
+  int block; unsigned grid;
+  XArgs<real> A = make_x<real>(c, &block, &grid);
+  A.u[0] = (const real*)c->cur[0]; A.u[1] = (const real*)c->cur[1];
+  A.bx = (const real*)c->cur[5]; A.by = (const real*)c->cur[6]; A.bz = (const real*)c->cur[7];
+  A.bxo = (real*)c->alt[5]; A.byo = (real*)c->alt[6]; A.bzo = (real*)c->alt[7];
+  A.t2_first = t2_first;
+  const size_t smem = (size_t)24 * block * sizeof(real);
+  static bool attr_set = false;
+  if (!attr_set) {
+    CUDA_TRY(c, cudaFuncSetAttribute(bpair_x_kernel<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, 24 * 256 * (int)sizeof(real)));
+    attr_set = true;
+  }
+  bpair_x_kernel<real><<<grid, block, smem, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  return MHD_OK;
+}
+
 template <class real>
 static int launch_fluid(mhd_ctx* c, int d) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
   if (c->n[d] == 1) return MHD_OK;   // both face fluxes of the only cell are identical: exact no-op (R10)
+  if (yz_ok(c, d)) return launch_fluid_yz<real>(c, d);
+  if (d == 0 && x_ok<real>(c)) return launch_fluid_x<real>(c);
   FluidArgs<real> A;
   const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
@@ -251,6 +386,8 @@ static int launch_fluid(mhd_ctx* c, int d) {
 template <class real>
 static int launch_bpair(mhd_ctx* c, int d, int t2_first) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  if (yz_ok(c, d)) return launch_bpair_yz<real>(c, d, t2_first);
+  if (d == 0 && x_ok<real>(c)) return launch_bpair_x<real>(c, t2_first);
   BPairArgs<real> A;
   A.rho = (const real*)c->cur[0]; A.md = (const real*)c->cur[1 + d];
   A.bd = (const real*)c->cur[5 + d]; A.bt1 = (const real*)c->cur[5 + t1]; A.bt2 = (const real*)c->cur[5 + t2];

@@ -2,6 +2,11 @@
 // PRODUCT code (CUDA path); shares nothing with oracle/.
 //
 // Citations are to /root/reference/PAPER.md (arxiv/paper_0908_4362), section 3.
+//
+// Arithmetic policy: the step is close to the ALU/issue roofline, so the
+// special functions are the cheap ones.  fp32: MUFU.RCP / MUFU.SQRT (rcp.approx.ftz, sqrt.approx.ftz,
+// <= 1-2 ulp, no slow path) -- far inside the 1e-5 per-step tolerance.  fp64: IEEE division and sqrt
+// (1e-12 tolerance).  No --use_fast_math: the discrete switches (a*b > 0, vh > 0) see IEEE products.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -18,47 +23,66 @@ __device__ __forceinline__ int map_index(int q, int n, int bc) {
   }
   return q < 0 ? 0 : (q >= n ? n - 1 : q);
 }
-
-template <class real> __device__ __forceinline__ real rabs(real x);
-template <> __device__ __forceinline__ float rabs<float>(float x) { return fabsf(x); }
-template <> __device__ __forceinline__ double rabs<double>(double x) { return fabs(x); }
-template <class real> __device__ __forceinline__ real rsqrt_(real x);
-template <> __device__ __forceinline__ float rsqrt_<float>(float x) { return sqrtf(x); }
-template <> __device__ __forceinline__ double rsqrt_<double>(double x) { return sqrt(x); }
-
-// van Leer limiter, eq (14); zero unless both half-differences have the same sign
-// (reading R8: strictly a*b > 0).
-template <class real>
-__device__ __forceinline__ real vanleer(real a, real b) {
-  const real ab = a * b;
-  return ab > real(0) ? (real(2) * ab) / (a + b) : real(0);
+// same, valid only for -n <= q < 2n (one wrap), branch free
+__device__ __forceinline__ int map_index1(int q, int n, int bc) {
+  if (bc == BC_PERIODIC) return q < 0 ? q + n : (q >= n ? q - n : q);
+  return q < 0 ? 0 : (q >= n ? n - 1 : q);
 }
 
-// Right- and left-going fluxes R = c u + F, G = c u - F (2c u^R and 2c u^L of eqs (9)-(10),
-// PAPER.md:85-89) for one cell.  u = (rho, m1, m2, m3, E) in sweep roles, b = cell-centred field
-// in sweep roles (held fixed).  F is eq (6), the freezing speed
-// c = |v| + sqrt(|gamma p + B^2| / rho) is PAPER.md:126.
+__device__ __forceinline__ float rcp_(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
+__device__ __forceinline__ float sqrt_(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+__device__ __forceinline__ float abs_(float x) { return fabsf(x); }
+__device__ __forceinline__ double abs_(double x) { return fabs(x); }
+
+// van Leer limiter of two HALF differences, eq (14), written for the FULL differences
+// a, b:  vanleer(a/2, b/2) = 2 (a/2)(b/2) / (a/2 + b/2) = a b / (a + b).  Zero unless a*b > 0
+// strictly (reading R8).
 template <class real>
-__device__ __forceinline__ void right_left(const real u[5], const real b[3], real gamma, real R[5], real G[5]) {
-  const real rho = u[0], m1 = u[1], m2 = u[2], m3 = u[3], E = u[4];
-  const real inv = real(1) / rho;
+__device__ __forceinline__ real vl_full(real a, real b) {
+  const real ab = a * b;
+  const real r = ab * rcp_(a + b);
+  return ab > real(0) ? r : real(0);
+}
+
+// Cell-centred field of one cell (held fixed through both stages) and what the two
+// flux evaluations need from it.
+template <class real>
+struct BCell {
+  real b0, b1, b2;   // sweep roles: b0 along the sweep
+  real hb2;          // |b|^2 / 2
+  __device__ __forceinline__ void set(real x, real y, real z) {
+    b0 = x; b1 = y; b2 = z;
+    hb2 = real(0.5) * (x * x + y * y + z * z);
+  }
+};
+
+// Right- and left-going fluxes R = c u + F, G = c u - F (2c u^R and 2c u^L of eqs (9)-(10),
+// PAPER.md:85-89) for one cell.  u = (rho, m1, m2, m3, E) in sweep roles.  F is eq (6) PAPER.md:76;
+// P* = P + B^2/2, P = (gamma-1)(E - rho v^2/2 - B^2/2); the freezing speed
+// c = |v| + sqrt(|gamma p + B^2| / rho) is PAPER.md:126 (|.|: reading R3).
+template <class real>
+__device__ __forceinline__ void right_left(const real u[5], const BCell<real>& B, real gamma, real R[5], real G[5]) {
+  const real m1 = u[1], m2 = u[2], m3 = u[3], E = u[4];
+  const real inv = rcp_(u[0]);
   const real v = m1 * inv;
-  const real b2 = b[0] * b[0] + b[1] * b[1] + b[2] * b[2];
-  const real ke = real(0.5) * (m1 * m1 + m2 * m2 + m3 * m3) * inv;
-  const real p = (gamma - real(1)) * (E - ke - real(0.5) * b2);
-  const real ps = p + real(0.5) * b2;
-  const real bdotv = (b[0] * m1 + b[1] * m2 + b[2] * m3) * inv;
+  const real ke2 = m1 * m1 + m2 * m2 + m3 * m3;
+  const real p = (gamma - real(1)) * ((E - B.hb2) - real(0.5) * (ke2 * inv));
+  const real ps = p + B.hb2;
+  const real bdotv = (B.b0 * m1 + B.b1 * m2 + B.b2 * m3) * inv;
   real F[5];
   F[0] = m1;
-  F[1] = m1 * v + ps - b[0] * b[0];
-  F[2] = m2 * v - b[1] * b[0];
-  F[3] = m3 * v - b[2] * b[0];
-  F[4] = (E + ps) * v - b[0] * bdotv;
-  const real c = rabs(v) + rsqrt_(rabs(gamma * p + b2) * inv);
+  F[1] = m1 * v + (ps - B.b0 * B.b0);
+  F[2] = m2 * v - B.b1 * B.b0;
+  F[3] = m3 * v - B.b2 * B.b0;
+  F[4] = (E + ps) * v - B.b0 * bdotv;
+  const real c = abs_(v) + sqrt_(abs_(gamma * p + real(2) * B.hb2) * inv);
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
-    R[k] = c * u[k] + F[k];
-    G[k] = c * u[k] - F[k];
+    const real cu = c * u[k];
+    R[k] = cu + F[k];
+    G[k] = cu - F[k];
   }
 }
 
@@ -66,77 +90,81 @@ __device__ __forceinline__ void right_left(const real u[5], const real b[3], rea
 template <class real>
 __device__ __forceinline__ real cfl_speed(real rho, real mx, real my, real mz, real E, real bx, real by, real bz,
                                           real gamma) {
-  const real inv = real(1) / rho;
+  const real inv = rcp_(rho);
   const real b2 = bx * bx + by * by + bz * bz;
   const real ke = real(0.5) * (mx * mx + my * my + mz * mz) * inv;
   const real p = (gamma - real(1)) * (E - ke - real(0.5) * b2);
-  const real vmax = fmax(fmax(rabs(mx * inv), rabs(my * inv)), rabs(mz * inv));
-  return vmax + rsqrt_(rabs(gamma * p + b2) * inv);
+  const real vmax = fmax(fmax(abs_(mx), abs_(my)), abs_(mz)) * inv;
+  return vmax + sqrt_(abs_(gamma * p + b2) * inv);
 }
 
 // ---------------------------------------------------------------------------------------------
 // Register pipeline of fluid_d for one pencil, fed one cell per call in sweep order.
 // Algorithm 1: first-order upwind half step eq (16), then the second-order TVD
 // full step eqs (11)-(15),(17) from u^{t+dt/2}.  After push() of cell q the updated u of cell q-3
-// is returned (valid once at least 7 cells have been pushed).
+// is returned (valid once 7 cells have been pushed).  Fluxes are carried as twice their value
+// (the 1/2 of  Phi = (R - G)/2  is folded into the dt factors).
 // ---------------------------------------------------------------------------------------------
 template <class real>
 struct FluidPipe {
   real u1_[5], u2_[5], u3_[5];   // u(q-1), u(q-2), u(q-3)
-  real bc1_[3];                  // B_c(q-1)
+  BCell<real> B1_;               // B_c(q-1)
   real R0_[5];                   // R of u^t at q-1
-  real phi1_[5];                 // first-order flux at face (q-2)+1/2
-  real Ra_[5], Rb_[5];           // R of u^{t+dt/2} at q-3, q-2
-  real Ga_[5], Gb_[5];           // G of u^{t+dt/2} at q-3, q-2
-  real Rp_[5];                   // limited right-going face value at (q-3)+1/2
-  real phi2_[5];                 // second-order flux at face (q-4)+1/2
+  real d1_[5];                   // 2 * first-order flux at face (q-2)+1/2
+  real Rb_[5], dRa_[5];          // R^{1}(q-2) and R^{1}(q-2) - R^{1}(q-3)          (R^{1}: from u^{t+dt/2})
+  real Gb_[5], dGa_[5];          // G^{1}(q-2) and G^{1}(q-3) - G^{1}(q-2)
+  real Rp_[5];                   // limited right-going value at face (q-3)+1/2
+  real phi2_[5];                 // 2 * second-order flux at face (q-4)+1/2
 
   __device__ __forceinline__ void init() {
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
       u1_[k] = u2_[k] = u3_[k] = real(1);
-      R0_[k] = phi1_[k] = Ra_[k] = Rb_[k] = Ga_[k] = Gb_[k] = Rp_[k] = phi2_[k] = real(0);
+      R0_[k] = d1_[k] = Rb_[k] = dRa_[k] = Gb_[k] = dGa_[k] = Rp_[k] = phi2_[k] = real(0);
     }
-    bc1_[0] = bc1_[1] = bc1_[2] = real(0);
+    B1_.set(real(0), real(0), real(0));
   }
 
-  // u, b: cell q.  out: updated u of cell q-3.
-  __device__ __forceinline__ void push(const real u[5], const real b[3], real gamma, real dt, real out[5]) {
+  // u, B: cell q.  out: updated u of cell q-3.  hdt = dt/2, qdt = dt/4.
+  __device__ __forceinline__ void push(const real u[5], const BCell<real>& B, real gamma, real hdt, real qdt, real out[5]) {
     real R0[5], G0[5];
-    right_left(u, b, gamma, R0, G0);                 // Alg. 1 step 4 at cell q
-    real uh[5], phi1[5];
+    right_left(u, B, gamma, R0, G0);                 // Alg. 1 step 4 at cell q
+    real uh[5], d1[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
-      phi1[k] = real(0.5) * (R0_[k] - G0[k]);        // step 5: first-order flux at face (q-1)+1/2
-      uh[k] = u1_[k] - (phi1[k] - phi1_[k]) * (dt * real(0.5));   // step 6: u^{t+dt/2}(q-1), eq (16)
+      d1[k] = R0_[k] - G0[k];                        // step 5: 2 * first-order flux at face (q-1)+1/2
+      uh[k] = u1_[k] - (d1[k] - d1_[k]) * qdt;       // step 6: u^{t+dt/2}(q-1), eq (16)
     }
     real Rc[5], Gc[5];
-    right_left(uh, bc1_, gamma, Rc, Gc);             // step 7 at cell q-1 (same B_c)
+    right_left(uh, B1_, gamma, Rc, Gc);              // step 7 at cell q-1 (same B_c)
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
       // step 8, eqs (11)-(15): right-going value at face (q-2)+1/2 from cells q-3,q-2,q-1;
-      // left-going value at face (q-3)+1/2 from cells q-3,q-2,q-1 (mirror image)
-      const real Rp = Rb_[k] + vanleer(real(0.5) * (Rb_[k] - Ra_[k]), real(0.5) * (Rc[k] - Rb_[k]));
-      const real Gp = Gb_[k] + vanleer(real(0.5) * (Gb_[k] - Gc[k]), real(0.5) * (Ga_[k] - Gb_[k]));
-      const real phi2 = real(0.5) * (Rp_[k] - Gp);   // flux at face (q-3)+1/2
-      out[k] = u3_[k] - (phi2 - phi2_[k]) * dt;      // step 9, eq (17) at cell q-3
+      // left-going value at face (q-3)+1/2 from the same cells (mirror image)
+      const real dRb = Rc[k] - Rb_[k];
+      const real Rp = Rb_[k] + vl_full(dRa_[k], dRb);
+      const real dGb = Gb_[k] - Gc[k];
+      const real Gp = Gb_[k] + vl_full(dGb, dGa_[k]);
+      const real phi2 = Rp_[k] - Gp;                 // 2 * flux at face (q-3)+1/2
+      out[k] = u3_[k] - (phi2 - phi2_[k]) * hdt;     // step 9, eq (17) at cell q-3
       // shift the window by one cell
       phi2_[k] = phi2;
       Rp_[k] = Rp;
-      Ra_[k] = Rb_[k]; Rb_[k] = Rc[k];
-      Ga_[k] = Gb_[k]; Gb_[k] = Gc[k];
-      phi1_[k] = phi1[k];
+      dRa_[k] = dRb; Rb_[k] = Rc[k];
+      dGa_[k] = dGb; Gb_[k] = Gc[k];
+      d1_[k] = d1[k];
       R0_[k] = R0[k];
       u3_[k] = u2_[k]; u2_[k] = u1_[k]; u1_[k] = u[k];
     }
-    bc1_[0] = b[0]; bc1_[1] = b[1]; bc1_[2] = b[2];
+    B1_ = B;
   }
 };
 
 // ---------------------------------------------------------------------------------------------
 // Register pipeline of B_{t->d} for one row of faces (Algorithm 2; eqs (20)-(22)
-// PAPER.md:147-158).  push(vt(q), B_t(q)) returns the second-order edge flux f*dt at face (q-4)+1/2;
-// flo() is the previous one (face (q-4)-1/2) and bold() is B_t(q-4).  Valid after 9 pushes.
+// PAPER.md:147-158).  push(vt(q), B_t(q)) produces the second-order edge flux f*dt at face
+// (q-4)+1/2 (fhi); flo() is the previous one (face (q-4)-1/2) and bold() is B_t(q-4).
+// Valid after 9 pushes.
 // ---------------------------------------------------------------------------------------------
 template <class real>
 struct BPipe {
@@ -146,24 +174,24 @@ struct BPipe {
   real f1_;               // first-order flux at face (q-3)+1/2
   real b1_, b2_, b3_, b4_;// B_t at q-1..q-4
   real wA_, wB_, wC_;     // vg*B_t^{t+dt/2} at q-5, q-4, q-3
-  real vhA_, vhB_;        // face velocity at (q-4)+1/2, (q-3)+1/2
+  real vhA_, vhB_;        // 2 * face velocity at (q-4)+1/2, (q-3)+1/2 (only the sign is used)
   real f_, flo_, bold_;
 
   __device__ __forceinline__ void init() {
     vt1_ = vt2_ = vg2_ = w02_ = f1_ = b1_ = b2_ = b3_ = b4_ = wA_ = wB_ = wC_ = vhA_ = vhB_ = f_ = flo_ = bold_ = real(0);
   }
 
-  __device__ __forceinline__ void push(real vt, real bt, real dt) {
+  __device__ __forceinline__ void push(real vt, real bt, real dt, real hdt) {
     const real vg1 = real(0.25) * ((vt2_ + vt) + real(2) * vt1_);      // eq (20) at q-1
     const real w01 = vg1 * b1_;
-    const real vh = real(0.5) * (vg2_ + vg1);                           // eq (22) at face (q-2)+1/2
+    const real vh = vg2_ + vg1;                                         // 2 * eq (22) at face (q-2)+1/2
     const real f1 = vh > real(0) ? w02_ : w01;                          // eq (21)
-    const real bh = b2_ - (f1 - f1_) * (dt * real(0.5));                // Alg. 2 step 7: B_t^{t+dt/2}(q-2)
+    const real bh = b2_ - (f1 - f1_) * hdt;                             // Alg. 2 step 7: B_t^{t+dt/2}(q-2)
     const real wD = vg2_ * bh;
-    // Alg. 2 step 8: second-order TVD flux at face (q-4)+1/2, upwinded by vhA_
+    // Alg. 2 step 8: second-order TVD flux at face (q-4)+1/2, upwinded by the sign of vhA_
     const bool up = vhA_ > real(0);
     const real x = up ? wB_ : wC_, y = up ? wA_ : wD, z = up ? wC_ : wB_;
-    const real f = x + vanleer(real(0.5) * (x - y), real(0.5) * (z - x));
+    const real f = x + vl_full(x - y, z - x);
     flo_ = f_;
     f_ = f * dt;
     bold_ = b4_;

@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(256) fluid_march_kernel(const FluidArgs<real> 
   int a, b, s;
   if (!thread_to_pencil(g, a, b, s)) return;
   const real dt = (real)(*A.dt);
+  const real hdt = real(0.5) * dt, qdt = real(0.25) * dt;
   const long long oab = a * g.sa + b * g.sb;
   const long long oa1 = map_index(a + 1, g.na, g.bc) * g.sa + b * g.sb;   // row a+1 (for B_t1 at its +face)
   const long long ob1 = a * g.sa + map_index(b + 1, g.nb, g.bc) * g.sb;   // row b+1 (for B_t2 at its +face)
@@ -68,16 +69,16 @@ __global__ void __launch_bounds__(256) fluid_march_kernel(const FluidArgs<real> 
   real bd_lo = A.bd[map_index(n0 - 3, g.nd, g.bc) * g.sd + oab];
   for (int q = n0 - 3; q < n1 + 3; ++q) {
     const long long od = map_index(q, g.nd, g.bc) * g.sd;
-    real u[5], bc[3];
+    real u[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) u[k] = A.u[k][od + oab];
     const real bd_hi = A.bd[map_index(q + 1, g.nd, g.bc) * g.sd + oab];
-    bc[0] = real(0.5) * (bd_lo + bd_hi);                               // eq (19): faces -> centre
-    bc[1] = real(0.5) * (A.bt1[od + oab] + A.bt1[od + oa1]);
-    bc[2] = real(0.5) * (A.bt2[od + oab] + A.bt2[od + ob1]);
+    BCell<real> B;                                                     // eq (19): faces -> centre
+    B.set(real(0.5) * (bd_lo + bd_hi), real(0.5) * (A.bt1[od + oab] + A.bt1[od + oa1]),
+          real(0.5) * (A.bt2[od + oab] + A.bt2[od + ob1]));
     bd_lo = bd_hi;
     real out[5];
-    pipe.push(u, bc, g.gamma, dt, out);
+    pipe.push(u, B, g.gamma, hdt, qdt, out);
     const int m = q - 3;
     if (m >= n0) {
       const long long o = (long long)m * g.sd + oab;
@@ -96,6 +97,7 @@ __global__ void __launch_bounds__(256) bpair_march_kernel(const BPairArgs<real> 
   int a, b, s;
   if (!thread_to_pencil(g, a, b, s)) return;
   const real dt = (real)(*A.dt);
+  const real hdt = real(0.5) * dt;
   const int am = map_index(a - 1, g.na, g.bc), ap = map_index(a + 1, g.na, g.bc);
   const int bm = map_index(b - 1, g.nb, g.bc), bp = map_index(b + 1, g.nb, g.bc);
   const long long o00 = a * g.sa + b * g.sb;
@@ -115,12 +117,12 @@ __global__ void __launch_bounds__(256) bpair_march_kernel(const BPairArgs<real> 
     const real rp0 = A.rho[od + op0], mp0 = A.md[od + op0];
     const real r0m = A.rho[od + o0m], m0m = A.md[od + o0m];
     const real r0p = A.rho[od + o0p], m0p = A.md[od + o0p];
-    p1.push((mm0 + m00) / (rm0 + r00), A.bt1[od + o00], dt);
-    p2.push((m0m + m00) / (r0m + r00), A.bt2[od + o00], dt);
+    p1.push((mm0 + m00) * rcp_(rm0 + r00), A.bt1[od + o00], dt, hdt);
+    p2.push((m0m + m00) * rcp_(r0m + r00), A.bt2[od + o00], dt, hdt);
     // the "+1" rows: row tau+1 uses cells map(tau), map(tau+1).  map(tau) = tau always; with clamping at
     // the last row map(tau+1) = tau too, so the same expression covers both boundary rules.
-    p1p.push((m00 + mp0) / (r00 + rp0), A.bt1[od + op0], dt);
-    p2p.push((m00 + m0p) / (r00 + r0p), A.bt2[od + o0p], dt);
+    p1p.push((m00 + mp0) * rcp_(r00 + rp0), A.bt1[od + op0], dt, hdt);
+    p2p.push((m00 + m0p) * rcp_(r00 + r0p), A.bt2[od + o0p], dt, hdt);
     const int m = q - 4;
     if (m >= n0) {
       const long long o = (long long)m * g.sd + o00;

@@ -48,13 +48,15 @@ def _ref_input(f, prec):
     return [np.array(np.asarray(a, dtype=dt), dtype=np.float64) for a in f]
 
 
-SHAPES = [(40, 24, 20), (48, 1, 1), (1, 40, 1), (1, 1, 36), (32, 20, 1), (1, 24, 16), (20, 1, 24), (7, 5, 3)]
+SHAPES = [(40, 24, 20), (48, 1, 1), (1, 40, 1), (1, 1, 36), (32, 20, 1), (1, 24, 16), (20, 1, 24), (7, 5, 3),
+          (136, 9, 8), (520, 3, 2), (64, 33, 1)]
 
 
+@pytest.mark.parametrize("path", [0, 1])          # 0: specialised x / yz kernels where they apply, 1: generic kernels only
 @pytest.mark.parametrize("shape", SHAPES)
 @pytest.mark.parametrize("bc", [P, O])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_each_operator_matches_oracle(B, shape, bc, prec):
+def test_each_operator_matches_oracle(B, shape, bc, prec, path):
     nx, ny, nz = shape
     f0 = random_state(nx, ny, nz, seed=nx * 7 + ny * 3 + nz + bc)
     gamma, dt = 5.0 / 3.0, 0.21
@@ -71,12 +73,12 @@ def test_each_operator_matches_oracle(B, shape, bc, prec):
                     oracle.badvect(ref, gamma, bc, d, t, dt)
             else:
                 oracle.sweep(ref, gamma, bc, d, op == B.MHD_OP_SWEEP_REVERSE, dt)
-            s = _solver(B, f0, gamma, bc, prec)
+            s = _solver(B, f0, gamma, bc, prec, path=path)
             s.apply(op, d, rev, dt)
             got = s.get_state()
             s.close()
             e = max_rel(got, ref)
-            assert worst(e) <= tol, (shape, bc, prec, d, op, rev, e)
+            assert worst(e) <= tol, (shape, bc, prec, d, op, rev, path, e)
 
 
 @pytest.mark.parametrize("seg", [0, 5, 13, 64])
