@@ -16,7 +16,7 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int, c_longlong, c_size
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmhd.so")
+LIB_PATH = os.environ.get("MHD_LIB") or os.path.join(_HERE, "libmhd.so")   # MHD_LIB: A/B-test another build of the same ABI
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(

@@ -33,6 +33,9 @@ struct mhd_ctx {
   bool owns_stream;
   bool stream_set;
   bool has_state;
+  bool acc_valid;          // the device accumulator cmax_bits holds c_max of the CURRENT state (fused reduction)
+  bool fin_valid;          // sc->cmax holds c_max of the current state
+  bool acc_dirty;          // the accumulator may be non-zero (must be zeroed before a new reduction starts)
   long long step_index;
   long long launches;
   // options
@@ -182,6 +185,7 @@ extern "C" int mhd_set_state(mhd_ctx* c, const void* const fields[8], int where)
   CUDA_TRY(c, cudaMemsetAsync(c->sc, 0, sizeof(Scalars), c->stream));
   if (where == MHD_HOST) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   c->has_state = true;
+  c->acc_valid = c->fin_valid = false;
   return MHD_OK;
 }
 
@@ -267,12 +271,13 @@ static dim3 yz_grid(const YZArgs<real>& A) {
 }
 
 template <class real>
-static int launch_fluid_yz(mhd_ctx* c, int d) {
+static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3, o = 3 - d;
   YZArgs<real> A = make_yz<real>(c, d);
   const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
+  A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
   fluid_yz_kernel<real, kYZBlock><<<yz_grid(A), kYZBlock, 0, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
@@ -321,12 +326,13 @@ static XArgs<real> make_x(mhd_ctx* c, int* block, unsigned* grid) {
 }
 
 template <class real>
-static int launch_fluid_x(mhd_ctx* c) {
+static int launch_fluid_x(mhd_ctx* c, bool want_cmax) {
   int block; unsigned grid;
   XArgs<real> A = make_x<real>(c, &block, &grid);
   const int role[5] = {0, 1, 2, 3, 4};
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
   A.bx = (const real*)c->cur[5]; A.by = (const real*)c->cur[6]; A.bz = (const real*)c->cur[7];
+  A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
   const size_t smem = (size_t)35 * block * sizeof(real);
   static bool attr_set = false;
   if (!attr_set) {
@@ -361,12 +367,15 @@ static int launch_bpair_x(mhd_ctx* c, int t2_first) {
   return MHD_OK;
 }
 
+// want_cmax: this is the last operator of a step; fuse the c_max reduction of the NEXT step into it.
+// *fused reports whether the kernel that ran could do so.
 template <class real>
-static int launch_fluid(mhd_ctx* c, int d) {
+static int launch_fluid(mhd_ctx* c, int d, bool want_cmax = false, bool* fused = nullptr) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  if (fused) *fused = false;
   if (c->n[d] == 1) return MHD_OK;   // both face fluxes of the only cell are identical: exact no-op (R10)
-  if (yz_ok(c, d)) return launch_fluid_yz<real>(c, d);
-  if (d == 0 && x_ok<real>(c)) return launch_fluid_x<real>(c);
+  if (yz_ok(c, d)) { if (fused) *fused = want_cmax; return launch_fluid_yz<real>(c, d, want_cmax); }
+  if (d == 0 && x_ok<real>(c)) { if (fused) *fused = want_cmax; return launch_fluid_x<real>(c, want_cmax); }
   FluidArgs<real> A;
   const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
@@ -424,14 +433,23 @@ static int launch_cfl(mhd_ctx* c) {
 
 #define BY_PRECISION(c, CALL32, CALL64) ((c)->precision == MHD_F32 ? (CALL32) : (CALL64))
 
-static int sweep(mhd_ctx* c, int d, bool reverse) {
+static int arm_accumulator(mhd_ctx* c) {
+  if (c->acc_dirty) {
+    CUDA_TRY(c, cudaMemsetAsync(&c->sc->cmax_bits, 0, sizeof(unsigned long long), c->stream));
+    c->acc_dirty = false;
+  }
+  return MHD_OK;
+}
+
+static int sweep(mhd_ctx* c, int d, bool reverse, bool want_cmax = false, bool* fused = nullptr) {
   int rc;
+  c->acc_valid = c->fin_valid = false;          // the state changes
   if (!reverse) {
     if ((rc = BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d)))) return rc;
     return BY_PRECISION(c, launch_bpair<float>(c, d, 0), launch_bpair<double>(c, d, 0));
   }
   if ((rc = BY_PRECISION(c, launch_bpair<float>(c, d, 1), launch_bpair<double>(c, d, 1)))) return rc;
-  return BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d));
+  return BY_PRECISION(c, launch_fluid<float>(c, d, want_cmax, fused), launch_fluid<double>(c, d, want_cmax, fused));
 }
 
 // one double sweep, eqs (23)-(25) PAPER.md:164-170
@@ -439,8 +457,14 @@ static int double_sweep(mhd_ctx* c) {
   static const int order[3][3] = {{0, 1, 2}, {2, 0, 1}, {1, 2, 0}};
   const int* o = order[((c->step_index % 3) + 3) % 3];
   int rc;
+  bool fused = false;
+  if ((rc = arm_accumulator(c))) return rc;
   for (int i = 0; i < 3; ++i) if ((rc = sweep(c, o[i], false))) return rc;
-  for (int i = 2; i >= 0; --i) if ((rc = sweep(c, o[i], true))) return rc;
+  // the last operator of the step (fluid of the reverse L along o[0]) also reduces c_max of the new
+  // state, so the next step needs no separate pass over the 8 fields
+  for (int i = 2; i >= 0; --i) if ((rc = sweep(c, o[i], true, i == 0, &fused))) return rc;
+  c->acc_valid = fused;
+  if (fused) c->acc_dirty = true;
   c->step_index++;
   return MHD_OK;
 }
@@ -451,15 +475,31 @@ static int read_scalars(mhd_ctx* c, Scalars* h) {
   return MHD_OK;
 }
 
+// make sc->cmax / sc->dt current: run the reduction only if no fused one is pending
+static int refresh_dt(mhd_ctx* c, double cfl, int advance) {
+  int reuse = 0;
+  if (c->fin_valid) reuse = 1;
+  else if (!c->acc_valid) {
+    int rc = arm_accumulator(c);
+    if (rc) return rc;
+    if ((rc = BY_PRECISION(c, launch_cfl<float>(c), launch_cfl<double>(c)))) return rc;
+    c->acc_dirty = true;
+  }
+  dt_from_cmax_kernel<<<1, 1, 0, c->stream>>>(c->sc, cfl, advance, reuse);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  if (!reuse) c->acc_dirty = false;            // finalising re-arms the accumulator
+  c->acc_valid = false;
+  c->fin_valid = true;
+  return MHD_OK;
+}
+
 extern "C" int mhd_cfl_dt(mhd_ctx* c, double cfl, double* dt_out, double* cmax_out) {
   if (!c) return MHD_EINVAL;
   if (!(cfl > 0.0) || !dt_out) return fail(c, MHD_EINVAL, "mhd_cfl_dt: bad argument");
   if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_cfl_dt: no state set");
-  int rc = BY_PRECISION(c, launch_cfl<float>(c), launch_cfl<double>(c));
+  int rc = refresh_dt(c, cfl, 0);
   if (rc) return rc;
-  dt_from_cmax_kernel<<<1, 1, 0, c->stream>>>(c->sc, cfl, 0);
-  c->launches++;
-  CUDA_TRY(c, cudaGetLastError());
   Scalars h;
   if ((rc = read_scalars(c, &h))) return rc;
   *dt_out = h.dt;
@@ -475,9 +515,7 @@ extern "C" int mhd_step(mhd_ctx* c, int n, double cfl, double* t_advanced) {
   reset_call_kernel<<<1, 1, 0, c->stream>>>(c->sc);
   c->launches++;
   for (int it = 0; it < n; ++it) {
-    if ((rc = BY_PRECISION(c, launch_cfl<float>(c), launch_cfl<double>(c)))) return rc;
-    dt_from_cmax_kernel<<<1, 1, 0, c->stream>>>(c->sc, cfl, 1);
-    c->launches++;
+    if ((rc = refresh_dt(c, cfl, 1))) return rc;
     if ((rc = double_sweep(c))) return rc;
   }
   CUDA_TRY(c, cudaGetLastError());
@@ -509,6 +547,7 @@ extern "C" int mhd_apply(mhd_ctx* c, int op, int d, int reverse, double dt) {
   if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_apply: no state set");
   set_dt_kernel<<<1, 1, 0, c->stream>>>(c->sc, dt, 0);
   c->launches++;
+  c->acc_valid = c->fin_valid = false;
   switch (op) {
     case MHD_OP_FLUID: return BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d));
     case MHD_OP_BPAIR:

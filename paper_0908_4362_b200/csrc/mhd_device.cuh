@@ -98,6 +98,28 @@ __device__ __forceinline__ real cfl_speed(real rho, real mx, real my, real mz, r
   return vmax + sqrt_(abs_(gamma * p + b2) * inv);
 }
 
+// same from sweep-role quantities: u = (rho, m1, m2, m3, E), hb2 = |B_c|^2 / 2
+template <class real>
+__device__ __forceinline__ real cfl_speed_hb2(const real u[5], real hb2, real gamma) {
+  const real inv = rcp_(u[0]);
+  const real ke = real(0.5) * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3]) * inv;
+  const real p = (gamma - real(1)) * (u[4] - ke - hb2);
+  const real vmax = fmax(fmax(abs_(u[1]), abs_(u[2])), abs_(u[3])) * inv;
+  return vmax + sqrt_(abs_(gamma * p + real(2) * hb2) * inv);
+}
+
+__device__ __forceinline__ unsigned long long speed_bits(float c) { return (unsigned long long)__double_as_longlong((double)c); }
+__device__ __forceinline__ unsigned long long speed_bits(double c) { return (unsigned long long)__double_as_longlong(c); }
+
+__device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+    v = w > v ? w : v;
+  }
+  return v;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Register pipeline of fluid_d for one pencil, fed one cell per call in sweep order.
 // Algorithm 1: first-order upwind half step eq (16), then the second-order TVD
@@ -109,6 +131,7 @@ template <class real>
 struct FluidPipe {
   real u1_[5], u2_[5], u3_[5];   // u(q-1), u(q-2), u(q-3)
   BCell<real> B1_;               // B_c(q-1)
+  real hb2_2_, hb2_3_;           // |B_c|^2/2 of cells q-2, q-3 (for the fused c_max reduction)
   real R0_[5];                   // R of u^t at q-1
   real d1_[5];                   // 2 * first-order flux at face (q-2)+1/2
   real Rb_[5], dRa_[5];          // R^{1}(q-2) and R^{1}(q-2) - R^{1}(q-3)          (R^{1}: from u^{t+dt/2})
@@ -123,7 +146,11 @@ struct FluidPipe {
       R0_[k] = d1_[k] = Rb_[k] = dRa_[k] = Gb_[k] = dGa_[k] = Rp_[k] = phi2_[k] = real(0);
     }
     B1_.set(real(0), real(0), real(0));
+    hb2_2_ = hb2_3_ = real(0);
   }
+  // |B_c|^2/2 of the cell whose update the last push() returned
+  __device__ __forceinline__ real hb2_out() const { return hb2_out_; }
+  real hb2_out_;
 
   // u, B: cell q.  out: updated u of cell q-3.  hdt = dt/2, qdt = dt/4.
   __device__ __forceinline__ void push(const real u[5], const BCell<real>& B, real gamma, real hdt, real qdt, real out[5]) {
@@ -156,6 +183,8 @@ struct FluidPipe {
       R0_[k] = R0[k];
       u3_[k] = u2_[k]; u2_[k] = u1_[k]; u1_[k] = u[k];
     }
+    hb2_out_ = hb2_3_;
+    hb2_3_ = hb2_2_; hb2_2_ = B1_.hb2;
     B1_ = B;
   }
 };

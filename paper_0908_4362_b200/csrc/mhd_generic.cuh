@@ -151,15 +151,6 @@ struct CflArgs {
   unsigned long long* cmax_bits;
 };
 
-__device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    const unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
-    v = w > v ? w : v;
-  }
-  return v;
-}
-
 template <class real>
 __global__ void __launch_bounds__(256) cfl_kernel(const CflArgs<real> A) {
   const long long N = (long long)A.nx * A.ny * A.nz;
@@ -204,10 +195,14 @@ struct Scalars {
 };
 
 // one thread: dt = cfl / c_max, t += 2 dt; re-arms the reduction
-__global__ void dt_from_cmax_kernel(Scalars* s, double cfl, int advance) {
-  const double cm = __longlong_as_double((long long)s->cmax_bits);
-  s->cmax = cm;
-  s->cmax_bits = 0ull;
+// reuse = 0: finalize the reduction (cmax <- accumulator, accumulator re-armed); 1: s->cmax is already final
+__global__ void dt_from_cmax_kernel(Scalars* s, double cfl, int advance, int reuse) {
+  double cm = s->cmax;
+  if (!reuse) {
+    cm = __longlong_as_double((long long)s->cmax_bits);
+    s->cmax = cm;
+    s->cmax_bits = 0ull;
+  }
   double dt = 0.0;
   if (!(cm > 0.0) || isinf(cm) || isnan(cm)) s->nonfinite = 1;
   else dt = cfl / cm;

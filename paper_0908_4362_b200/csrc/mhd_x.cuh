@@ -43,6 +43,7 @@ struct XArgs {
   const real *bx, *by, *bz;
   real *bxo, *byo, *bzo;
   const double* dt;
+  unsigned long long* cmax_bits;   // != nullptr: also reduce c of eq (18) over the updated cells
   int nx, ny, nz;
   int tpr;                 // threads per row = nx / V
   int rpb;                 // rows per block
@@ -149,13 +150,24 @@ __global__ void __launch_bounds__(256) fluid_x_kernel(const XArgs<real> A) {
   }
   __syncthreads();
   // step 9: full step (eq (17)) and store
+  real un[V][5];
 #pragma unroll
   for (int c = 0; c < 5; ++c) {
     phi[0][c] = S(6, c, tl);
     real o[V];
 #pragma unroll
-    for (int v = 0; v < V; ++v) o[v] = u[c][v] - (phi[v + 1][c] - phi[v][c]) * hdt;
+    for (int v = 0; v < V; ++v) { o[v] = u[c][v] - (phi[v + 1][c] - phi[v][c]) * hdt; un[v][c] = o[v]; }
     if (live) vstore(A.uo[c] + off, o);
+  }
+  if (A.cmax_bits) {            // last operator of a step: c of eq (18) from the updated cells (B unchanged)
+    unsigned long long cbest = 0ull;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const unsigned long long b = speed_bits(cfl_speed_hb2(un[v], B[v].hb2, A.gamma));
+      cbest = b > cbest ? b : cbest;
+    }
+    cbest = warp_max_u64(live ? cbest : 0ull);
+    if ((tid & 31) == 0) atomicMax(A.cmax_bits, cbest);
   }
 }
 

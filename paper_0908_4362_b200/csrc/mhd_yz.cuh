@@ -52,13 +52,26 @@ __device__ __forceinline__ void load_fluid(const YZArgs<real>& A, int q, int bas
 }
 
 // fluid_y / fluid_z, Algorithm 1
+#ifndef MHD_YZ_MINB
+#define MHD_YZ_MINB 4
+#endif
+#ifndef MHD_YZ_UNROLL
+#define MHD_YZ_UNROLL 3
+#endif
+#ifndef MHD_YZ_PREFETCH
+#define MHD_YZ_PREFETCH 1
+#endif
+#define MHD_STR2(x) #x
+#define MHD_STR(x) MHD_STR2(x)
+
 template <class real, int BLOCK>
-__global__ void __launch_bounds__(BLOCK) fluid_yz_kernel(const YZArgs<real> A) {
-  const int i = blockIdx.x * BLOCK + threadIdx.x;
-  if (i >= A.nx) return;
+__global__ void __launch_bounds__(BLOCK, MHD_YZ_MINB) fluid_yz_kernel(const YZArgs<real> A) {
+  int i = blockIdx.x * BLOCK + threadIdx.x;
+  const bool live = i < A.nx;
+  if (!live) i = A.nx - 1;                     // stay in step for the warp reduction; stores are masked
   const int o = blockIdx.y;
   const int n0 = blockIdx.z * A.seg;
-  const int n1 = min(n0 + A.seg, A.nd);
+  const int n1 = live ? min(n0 + A.seg, A.nd) : n0 - 6;   // dead threads run no iteration
   const real dt = (real)(*A.dt);
   const real hdt = real(0.5) * dt, qdt = real(0.25) * dt;
   const int base = i + o * A.so;
@@ -71,26 +84,38 @@ __global__ void __launch_bounds__(BLOCK) fluid_yz_kernel(const YZArgs<real> A) {
   FluidIn<real> cur, nxt;
   load_fluid(A, n0 - 3, base, xp_off, op_off, cur);
   unsigned long long cbest = 0ull;
-#pragma unroll 2
+_Pragma(MHD_STR(unroll MHD_YZ_UNROLL))
   for (int q = n0 - 3; q < n1 + 3; ++q) {
+#if MHD_YZ_PREFETCH
     if (q + 1 < n1 + 3) load_fluid(A, q + 1, base, xp_off, op_off, nxt);   // prefetch the next cell
+#else
+    if (q > n0 - 3) load_fluid(A, q, base, xp_off, op_off, cur);
+#endif
     BCell<real> B;                                                           // eq (19): faces -> centre
     const real bxc = real(0.5) * (cur.bxa + cur.bxb), boc = real(0.5) * (cur.boa + cur.bob);
     if (A.x_is_t1) B.set(real(0.5) * (bd_lo + cur.bd_hi), bxc, boc);
     else           B.set(real(0.5) * (bd_lo + cur.bd_hi), boc, bxc);
     bd_lo = cur.bd_hi;
     real out[5];
-    // B of cell q-3 is needed for the fused CFL reduction; keep what push() is about to shift out
     pipe.push(cur.u, B, A.gamma, hdt, qdt, out);
     const int m = q - 3;
     if (m >= n0) {
       const int off = m * A.sd + base;
 #pragma unroll
       for (int k = 0; k < 5; ++k) A.uo[k][off] = out[k];
+      if (A.cmax_bits) {          // last operator of a step: c of eq (18) from the updated cell (B unchanged)
+        const unsigned long long b = speed_bits(cfl_speed_hb2(out, pipe.hb2_out(), A.gamma));
+        cbest = b > cbest ? b : cbest;
+      }
     }
+#if MHD_YZ_PREFETCH
     cur = nxt;
+#endif
   }
-  (void)cbest;
+  if (A.cmax_bits) {
+    cbest = warp_max_u64(cbest);
+    if ((threadIdx.x & 31) == 0) atomicMax(A.cmax_bits, cbest);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -285,3 +285,40 @@ def test_uniform_state_fixed_point_and_empty_step_count(B):
     s.close()
     for a, b in zip(f, got):
         assert np.array_equal(a, b)
+
+
+def test_fused_cfl_reduction_paths(B):
+    """the c_max of step k+1 is reduced inside the last fluid kernel of step k: every way of reaching
+    a dt (fresh reduction, pending fused accumulator, finalised value, invalidation by mhd_apply)
+    must agree with the oracle"""
+    f, meta = inputs.turbulence(40, 32, 24)
+    gamma, bc = meta["gamma"], meta["bc"]
+    ref = _ref_input(f, "f64")
+    s = _solver(B, f, gamma, bc, "f64")
+    t_ref = oracle.run(ref, gamma, bc, 0, 7, 0.8)          # all three rotations end in a different fluid kernel
+    t = s.step(7, 0.8)
+    assert abs(t - t_ref) <= 1e-12 * t_ref
+    assert worst(max_rel(s.get_state(), ref)) <= 7 * TOL64
+    # pending fused accumulator -> cfl_dt without a new reduction
+    dt, cm = s.cfl_dt(0.8)
+    assert abs(cm - oracle.cmax(ref, gamma, bc)) <= 1e-13 * cm
+    # finalised value reused by the next step
+    t_ref = oracle.run(ref, gamma, bc, 7, 2, 0.8)
+    t = s.step(2, 0.8)
+    assert abs(t - t_ref) <= 1e-12 * t_ref
+    # step_fixed leaves a valid accumulator of the LAST state only
+    oracle.step_fixed(ref, gamma, bc, 9, 0.05)
+    oracle.step_fixed(ref, gamma, bc, 10, 0.05)
+    s.step_fixed(2, 0.05)
+    dt, cm = s.cfl_dt(0.8)
+    assert abs(cm - oracle.cmax(ref, gamma, bc)) <= 1e-13 * cm
+    # a single operator invalidates everything
+    oracle.fluid(ref, gamma, bc, 1, 0.05)
+    s.apply(B.MHD_OP_FLUID, 1, 0, 0.05)
+    dt, cm = s.cfl_dt(0.8)
+    assert abs(cm - oracle.cmax(ref, gamma, bc)) <= 1e-13 * cm
+    t_ref = oracle.run(ref, gamma, bc, 11, 3, 0.8)
+    t = s.step(3, 0.8)
+    assert abs(t - t_ref) <= 1e-12 * t_ref
+    assert worst(max_rel(s.get_state(), ref)) <= 20 * TOL64
+    s.close()
