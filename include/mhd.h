@@ -112,7 +112,10 @@ int mhd_get_time(mhd_ctx* ctx, double* t);
 int mhd_diagnostics(mhd_ctx* ctx, double sums[8], double* max_abs_divb);
 
 /* Tuning knobs, all optional: key "segment" = cells per thread along the sweep for the marching
- * kernels (0 = whole pencil), "block" = threads per block, "path" = 0 auto | 1 generic kernels only.
+ * kernels (0 = whole pencil), "block" = threads per block of the generic kernels, "path" = 0 auto |
+ * 1 generic kernels only, "btile" = tile shape of the y/z B-pair kernel (0 off, 1 = 32x8 default, 2 = 64x8,
+ * 3 = 64x4, 4 = 128x4), "ftma" = stages of the TMA bulk-copy ring of the y/z fluid kernel (0 off, 4, 6
+ * default, 8).
  * Unknown keys return MHD_EINVAL. */
 int mhd_set_option(mhd_ctx* ctx, const char* key, long long value);
 

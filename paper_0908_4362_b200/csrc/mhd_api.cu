@@ -11,6 +11,8 @@
 #include "mhd_generic.cuh"
 #include "mhd_yz.cuh"
 #include "mhd_x.cuh"
+#include "mhd_btile.cuh"
+#include "mhd_yz_tma.cuh"
 
 using namespace mhd;
 
@@ -39,7 +41,7 @@ struct mhd_ctx {
   long long step_index;
   long long launches;
   // options
-  int opt_segment, opt_block, opt_path;
+  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma;
   int sm_count;
   char err[512];
 };
@@ -101,6 +103,8 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_segment = -1;   // auto
   c->opt_block = 128;
   c->opt_path = 0;
+  c->opt_btile = 1;
+  c->opt_ftma = 8;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -278,6 +282,18 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
+  // TMA bulk-copy ring (mhd_yz_tma.cuh) when rows are whole 16-byte aligned blocks, else register prefetch
+  const int D = c->opt_ftma;
+  const int TXB = A.nx % 128 == 0 ? 128 : (A.nx % 32 == 0 ? 32 : 0);
+  if (D && TXB && (A.nx * sizeof(real)) % 16 == 0) {
+    const dim3 grid(A.nx / TXB, A.no, (A.nd + A.seg - 1) / A.seg);
+    void (*k)(const YZArgs<real>) = nullptr;
+    size_t smem = 0;
+    if (TXB == 128) { smem = FluidRing<real, 128>::smem_bytes(D); k = D == 4 ? fluid_yz_tma_kernel<real, 128, 4> : (D == 8 ? fluid_yz_tma_kernel<real, 128, 8> : fluid_yz_tma_kernel<real, 128, 6>); }
+    else            { smem = FluidRing<real, 32>::smem_bytes(D);  k = D == 4 ? fluid_yz_tma_kernel<real, 32, 4>  : (D == 8 ? fluid_yz_tma_kernel<real, 32, 8>  : fluid_yz_tma_kernel<real, 32, 6>); }
+    CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k<<<grid, TXB + 32, smem, c->stream>>>(A);
+  } else
   fluid_yz_kernel<real, kYZBlock><<<yz_grid(A), kYZBlock, 0, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
@@ -293,6 +309,18 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];
   A.t2_first = t2_first;
+  // tile march (mhd_btile.cuh) when the transverse extents tile evenly, else one thread per pencil
+  const int tshape[5][2] = {{0, 0}, {32, 8}, {64, 8}, {64, 4}, {128, 4}};
+  const int TXs = tshape[c->opt_btile][0], TOs = tshape[c->opt_btile][1];
+  if (TXs && A.nx % TXs == 0 && A.no % TOs == 0) {
+    const dim3 grid(A.nx / TXs, A.no / TOs, (A.nd + A.seg - 1) / A.seg);
+    switch (c->opt_btile) {
+      case 1: bpair_tile_kernel<real, 32, 8><<<grid, 9 * 32, 0, c->stream>>>(A); break;
+      case 2: bpair_tile_kernel<real, 64, 8><<<grid, 9 * 64, 0, c->stream>>>(A); break;
+      case 3: bpair_tile_kernel<real, 64, 4><<<grid, 5 * 64, 0, c->stream>>>(A); break;
+      default: bpair_tile_kernel<real, 128, 4><<<grid, 5 * 128, 0, c->stream>>>(A); break;
+    }
+  } else
   bpair_yz_kernel<real, kYZBlock><<<yz_grid(A), kYZBlock, 0, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
@@ -616,6 +644,8 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
     if (value < 32 || value > 256 || (value & 31)) return fail(c, MHD_EINVAL, "block must be a multiple of 32 in [32,256]");
     c->opt_block = (int)value; return MHD_OK;
   }
+  if (!strcmp(key, "ftma")) { if (value != 0 && value != 4 && value != 6 && value != 8) return fail(c, MHD_EINVAL, "ftma must be 0, 4, 6 or 8"); c->opt_ftma = (int)value; return MHD_OK; }
+  if (!strcmp(key, "btile")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btile must be 0..4"); c->opt_btile = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
   return fail(c, MHD_EINVAL, "unknown option '%s'", key);
 }

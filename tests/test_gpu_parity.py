@@ -49,7 +49,7 @@ def _ref_input(f, prec):
 
 
 SHAPES = [(40, 24, 20), (48, 1, 1), (1, 40, 1), (1, 1, 36), (32, 20, 1), (1, 24, 16), (20, 1, 24), (7, 5, 3),
-          (136, 9, 8), (520, 3, 2), (64, 33, 1)]
+          (136, 9, 8), (520, 3, 2), (64, 33, 1), (64, 16, 16), (32, 8, 24)]
 
 
 @pytest.mark.parametrize("path", [0, 1])          # 0: specialised x / yz kernels where they apply, 1: generic kernels only
@@ -322,3 +322,26 @@ def test_fused_cfl_reduction_paths(B):
     assert abs(t - t_ref) <= 1e-12 * t_ref
     assert worst(max_rel(s.get_state(), ref)) <= 20 * TOL64
     s.close()
+
+
+@pytest.mark.parametrize("btile", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("bc", [P, O])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_b_pair_tile_shapes(B, btile, bc, prec):
+    """every tile shape of the y/z tile-march B kernel (and the per-pencil kernel, btile = 0), with segments"""
+    f0 = random_state(128, 16, 24, seed=77 + bc)
+    gamma, dt = 5.0 / 3.0, 0.19
+    tol = TOL64 if prec == "f64" else TOL32_STEP
+    for d in (1, 2):
+        for rev in (0, 1):
+            ref = _ref_input(f0, prec)
+            t1, t2 = (d + 1) % 3, (d + 2) % 3
+            for t in ((t2, t1) if rev else (t1, t2)):
+                oracle.badvect(ref, gamma, bc, d, t, dt)
+            for seg in (0, 9):
+                s = _solver(B, f0, gamma, bc, prec, btile=btile, segment=seg)
+                s.apply(B.MHD_OP_BPAIR, d, rev, dt)
+                got = s.get_state()
+                s.close()
+                e = max_rel(got, ref)
+                assert worst(e) <= tol, (btile, bc, prec, d, rev, seg, e)
