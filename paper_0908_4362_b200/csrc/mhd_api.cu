@@ -13,6 +13,7 @@
 #include "mhd_x.cuh"
 #include "mhd_btile.cuh"
 #include "mhd_yz_tma.cuh"
+#include "mhd_btma.cuh"
 
 using namespace mhd;
 
@@ -41,7 +42,7 @@ struct mhd_ctx {
   long long step_index;
   long long launches;
   // options
-  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma;
+  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages;
   int sm_count;
   char err[512];
 };
@@ -105,6 +106,8 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_path = 0;
   c->opt_btile = 1;
   c->opt_ftma = 8;
+  c->opt_btma = 1;
+  c->opt_bstages = 6;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -309,6 +312,34 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];
   A.t2_first = t2_first;
+  // TMA-fed tile march (mhd_btma.cuh) when rows are whole 16-byte aligned blocks and the extents tile evenly
+  {
+    static const int shp[5][2] = {{0, 0}, {32, 8}, {64, 4}, {128, 2}, {64, 8}};
+    const int TXs = shp[c->opt_btma][0], TOs = shp[c->opt_btma][1];
+    if (TXs && A.nx % TXs == 0 && A.no % TOs == 0 && (A.nx * sizeof(real)) % 16 == 0) {
+      const dim3 grid(A.nx / TXs, A.no / TOs, (A.nd + A.seg - 1) / A.seg);
+      const int D = c->opt_bstages;
+      void (*k)(const YZArgs<real>) = nullptr;
+      size_t smem = 0;
+      int nthr = 0;
+#define MHD_BTMA_CASE(ID, TX_, TO_)                                                                         \
+      case ID: smem = BRing<real, TX_, TO_>::smem_bytes(D); nthr = BRing<real, TX_, TO_>::NT + 32;            \
+        k = D == 4 ? bpair_tma_kernel<real, TX_, TO_, 4> : (D == 8 ? bpair_tma_kernel<real, TX_, TO_, 8> : bpair_tma_kernel<real, TX_, TO_, 6>); break;
+      switch (c->opt_btma) {
+        MHD_BTMA_CASE(1, 32, 8)
+        MHD_BTMA_CASE(2, 64, 4)
+        MHD_BTMA_CASE(3, 128, 2)
+        default: MHD_BTMA_CASE(4, 64, 8)
+      }
+#undef MHD_BTMA_CASE
+      CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k<<<grid, nthr, smem, c->stream>>>(A);
+      c->launches++;
+      CUDA_TRY(c, cudaGetLastError());
+      for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+      return MHD_OK;
+    }
+  }
   // tile march (mhd_btile.cuh) when the transverse extents tile evenly, else one thread per pencil
   const int tshape[5][2] = {{0, 0}, {32, 8}, {64, 8}, {64, 4}, {128, 4}};
   const int TXs = tshape[c->opt_btile][0], TOs = tshape[c->opt_btile][1];
@@ -645,6 +676,8 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
     c->opt_block = (int)value; return MHD_OK;
   }
   if (!strcmp(key, "ftma")) { if (value != 0 && value != 4 && value != 6 && value != 8) return fail(c, MHD_EINVAL, "ftma must be 0, 4, 6 or 8"); c->opt_ftma = (int)value; return MHD_OK; }
+  if (!strcmp(key, "btma")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btma must be 0..4"); c->opt_btma = (int)value; return MHD_OK; }
+  if (!strcmp(key, "bstages")) { if (value != 4 && value != 6 && value != 8) return fail(c, MHD_EINVAL, "bstages must be 4, 6 or 8"); c->opt_bstages = (int)value; return MHD_OK; }
   if (!strcmp(key, "btile")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btile must be 0..4"); c->opt_btile = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
   return fail(c, MHD_EINVAL, "unknown option '%s'", key);

@@ -5,110 +5,203 @@
 // of the cells i-1 and o-1.  Instead of every thread recomputing its neighbours' flux pipelines and
 // re-reading their rho, m_d from global memory (mhd_yz.cuh: 4 pipelines, 15 loads per cell), a block
 // owns a TX x TO tile of pencils in the (x, o) plane and marches along d in lock step:
-//   * every thread runs only its own two pipelines (B_x row i, B_o row o),
+//   * every thread loads only its own cell (rho, m_d, B_x, B_o, B_d: 5 coalesced loads, prefetched one
+//     march step ahead) and runs only its own two pipelines (B_x row i, B_o row o),
 //   * rho, m_d and the finished fluxes are exchanged through double-buffered shared memory with one
-//     __syncthreads per march step,
+//     block barrier per march step,
 //   * one extra "halo" row of threads runs the B_o pipelines of row o0+TO and, in its first TO lanes,
-//     the B_x pipelines of column x0+TX, so nothing else is recomputed (overhead 1/TO).
-// Per cell: 5 global loads (rho, m_d, B_x, B_o, B_d) + 3 stores, 2 pipelines.
+//     the B_x pipelines of column x0+TX; its next TO lanes fetch column x0-1 (overhead 1/TO).
+// The loop is unrolled by 4 with the pipeline state held in circular register arrays (BPipe4), so the
+// delay lines cost no register moves: ncu on the first version of this kernel showed 264 instructions
+// per cell of which 46 were moves and ~100 address arithmetic (profiles/r01_c4_step_ncu_full.md).
 //
 // Requirements (else bpair_yz_kernel runs): nx % TX == 0, no % TO == 0, extent along the sweep >= 8.
 #pragma once
+#include <type_traits>
 #include "mhd_yz.cuh"
 
 namespace mhd {
 
-template <class real, int TX, int TO>
-__global__ void __launch_bounds__((TO + 1) * TX) bpair_tile_kernel(const YZArgs<real> A) {
-  static_assert(TO <= 32 && TX % 32 == 0, "tile shape");
-  constexpr int TW = TX + 2, TH = TO + 2;
-  __shared__ real sR[2][TH * TW], sM[2][TH * TW];      // rho, m_d at tile coords (o_local+1, x_local+1)
-  __shared__ real sFX[2][TO * (TX + 1) + 1];           // B_x-row fluxes at (o_local, x_local), x_local <= TX; +1 dummy
-  __shared__ real sFO[2][(TO + 1) * TX];               // B_o-row fluxes at (o_local <= TO, x_local)
+// Register pipeline of B_{t->d} for one row of faces (Algorithm 2; eqs (20)-(22)
+// PAPER.md:147-158) with all delay lines as circular arrays indexed by the march step modulo 4 (K is a
+// compile-time constant inside the 4x unrolled loop).  push<K>(vt(k), B_t(k)) finishes the second-order
+// edge flux f*dt at face (k-4)+1/2 and returns B_t'(k-4); flo is the flux at face (k-4)-1/2, fhi the new one.
+template <class real>
+struct BPipe4 {
+  real vt[2];        // vt(k-2), vt(k-1)            slot = step & 1
+  real b[4];         // B_t(k-4..k-1)               slot = step & 3
+  real w1[4];        // vg*B_t^{t+dt/2}(k-5..k-2)    slot = step & 3
+  real vh[2];        // 2 * face velocity at (k-4)+1/2, (k-3)+1/2 (only the sign is used)
+  real vg, w0, f1, f;   // vg(k-2), vg*B_t(k-2), first-order flux at (k-3)+1/2, second-order flux*dt at (k-5)+1/2
 
-  const int tid = threadIdx.x;
-  const int row = tid / TX, col = tid - row * TX;
-  const bool halo = row == TO;
+  __device__ __forceinline__ void init() {
+    vt[0] = vt[1] = vh[0] = vh[1] = vg = w0 = f1 = f = real(0);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = w1[j] = real(0);
+  }
+  __device__ __forceinline__ real fhi() const { return f; }     // after push: flux*dt at face (k-4)+1/2
+
+  template <int K>
+  __device__ __forceinline__ void push(real vtn, real btn, real dt, real hdt, real& bnew, real& flo) {
+    const real vg1 = real(0.25) * ((vt[K & 1] + vtn) + real(2) * vt[(K + 1) & 1]);   // eq (20) at k-1
+    const real w01 = vg1 * b[(K + 3) & 3];
+    const real vh2 = vg + vg1;                                                       // 2 * eq (22) at face (k-2)+1/2
+    const real f1n = vh2 > real(0) ? w0 : w01;                                       // eq (21)
+    const real bh = b[(K + 2) & 3] - (f1n - f1) * hdt;                               // Alg. 2 step 7: B_t^{t+dt/2}(k-2)
+    const real wD = vg * bh;
+    // Alg. 2 step 8: second-order TVD flux at face (k-4)+1/2, upwinded by the sign of the face velocity there
+    const bool up = vh[K & 1] > real(0);
+    const real wA = w1[(K + 3) & 3], wB = w1[K & 3], wC = w1[(K + 1) & 3];           // at k-5, k-4, k-3
+    const real x = up ? wB : wC, y = up ? wA : wD, z = up ? wC : wB;
+    const real fn = (x + vl_full(x - y, z - x)) * dt;
+    bnew = b[K & 3] - (fn - f);                                                      // Alg. 2 step 9 at cell k-4
+    flo = f;
+    f = fn; f1 = f1n; vg = vg1; w0 = w01;
+    vt[K & 1] = vtn; b[K & 3] = btn; w1[(K + 2) & 3] = wD; vh[K & 1] = vh2;
+  }
+};
+
+template <class real, int TX, int TO>
+struct BTile {
+  static constexpr int TW = TX + 2, TH = TO + 2;
+  static constexpr int NU = TH * TW;                     // rho / m_d tile incl. one-cell halo, slot (o_local+1)*TW + x_local+1
+  static constexpr int NFX = TO * (TX + 1) + 1;          // B_x-row fluxes at (o_local, x_local <= TX); +1 dummy
+  static constexpr int NFO = (TO + 1) * TX;              // B_o-row fluxes at (o_local <= TO, x_local)
+  static constexpr int BUF = 2 * NU + NFX + NFO;         // reals per buffer
+  static constexpr int NT = (TO + 1) * TX;
+};
+
+// keeps a per-thread constant in a register: without it ptxas rematerialises these few-instruction
+// index expressions inside the march loop, every step
+__device__ __forceinline__ void pin_reg(int& v) { asm volatile("" : "+r"(v)); }
+
+#ifndef MHD_BTILE_MINB
+#define MHD_BTILE_MINB 3
+#endif
+
+// One thread's march.  ROLE 0: interior tile rows 1..TO-1; 1: tile row 0 (also fetches row o0-1);
+// 2: the halo row.  Roles are warp uniform, so every warp runs exactly one instantiation; all of them
+// meet at the same hardware barrier (bar.sync 0) once per march step.
+template <class real, int TX, int TO, int ROLE>
+__device__ __forceinline__ void bpair_tile_march(const YZArgs<real>& A, real* sm, const int row, const int col) {
+  using T = BTile<real, TX, TO>;
+  constexpr int TW = T::TW;
+  constexpr bool halo = ROLE == 2;
   const int x0 = blockIdx.x * TX, o0 = blockIdx.y * TO;
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
   const real dt = (real)(*A.dt);
   const real hdt = real(0.5) * dt;
 
-  // ---- where my two pipelines sit (global, index-mapped) and where they live in the tiles --------
-  const int iO = x0 + col;
+  // my O position (B_o pipeline; rho, m_d, B_d of my own cell) and X position (B_x pipeline).
+  // interior thread: both are my cell.  halo row: O = (x0+col, o0+TO); X = lanes < TO: (x0+TX, o0+col),
+  // lanes TO..2TO-1: (x0-1, o0+col-TO) (fetch only), other lanes idle in the X role.
+  const int xrole = !halo ? 0 : (col < TO ? 1 : (col < 2 * TO ? 2 : 3));
   const int oO = halo ? map_index1(o0 + TO, A.no, A.bc) : o0 + row;
-  const bool hasX = !halo || col < TO;
-  const int iX = halo ? map_index1(x0 + TX, A.nx, A.bc) : iO;
-  const int oX = halo ? o0 + (hasX ? col : 0) : oO;
-  const int offO = iO + oO * A.so, offX = iX + oX * A.so;
-  const int tO = (halo ? TO + 1 : row + 1) * TW + col + 1;          // tile slot of the O position
-  const int tX = halo ? (hasX ? (col + 1) * TW + TX + 1 : tO) : tO;  // tile slot of the X position
-  const int nbX = tX - 1;                                            // cell x-1 of the X pipeline
-  const int nbO = tO - TW;                                           // cell o-1 of the O pipeline
-  const int fXw = halo ? (hasX ? col * (TX + 1) + TX : TO * (TX + 1)) : row * (TX + 1) + col;   // dummy slot for idle lanes
-  const int fOw = (halo ? TO : row) * TX + col;
-  const int fXr = row * (TX + 1) + col + 1, fOr = (row + 1) * TX + col;      // interior only
-  // extra tile cells loaded by interior threads: row o0-1 (by row 0) and column x0-1 (by column 0)
-  const bool exR = !halo && row == 0, exC = !halo && col == 0;
-  const int offR = iO + map_index1(o0 - 1, A.no, A.bc) * A.so;
-  const int offC = map_index1(x0 - 1, A.nx, A.bc) + oO * A.so;
-  const int tR = col + 1, tC = (row + 1) * TW;
+  int offO = x0 + col + oO * A.so;
+  const int xr_row = xrole == 2 ? col - TO : (xrole == 1 ? col : 0);
+  const int iX = xrole == 1 ? map_index1(x0 + TX, A.nx, A.bc) : map_index1(x0 - 1, A.nx, A.bc);
+  int offX = halo ? iX + (o0 + xr_row) * A.so : offO;                  // halo: my X cell; row 0: the cell in row o0-1
+  if (ROLE == 1) offX = x0 + col + map_index1(o0 - 1, A.no, A.bc) * A.so;
+  // tile slots (in reals, relative to the buffer)
+  int tO = (halo ? TO + 1 : row + 1) * TW + col + 1;
+  int tX = xrole == 1 ? (xr_row + 1) * TW + TX + 1 : (xrole == 2 ? (xr_row + 1) * TW : (ROLE == 1 ? col + 1 : tO));
+  int fXw = T::NU * 2 + (halo ? (xrole == 1 ? xr_row * (TX + 1) + TX : TO * (TX + 1)) : row * (TX + 1) + col);
+  int fOw = T::NU * 2 + T::NFX + (halo ? TO : row) * TX + col;
+  pin_reg(offO); pin_reg(offX); pin_reg(tO); pin_reg(tX); pin_reg(fXw); pin_reg(fOw);
+  const int nbO = tO - TW;                                            // cell o-1 of the O pipeline
+  const int nbX = (halo ? tX : tO) - 1;                               // cell x-1 of the X pipeline
+  const int fXr = fXw + 1, fOr = fOw + TX;                            // interior only: the rows i+1 and o+1
+  const bool xload = xrole <= 2;                                      // halo: fetches rho, m_d, B_x at its X cell
+  const bool x_first = (A.x_is_t1 != 0) != (A.t2_first != 0);         // forward: t1 then t2; reverse: t2 then t1
 
   const real* __restrict__ rho = A.u[0];
   const real* __restrict__ md = A.u[1];
+  const real* __restrict__ bxp = A.bx;
+  const real* __restrict__ bop = A.bo;
+  const real* __restrict__ bdp = A.bd;
 
-  struct In { real rO, mO, rX, mX, rE, mE, rF, mF, bX, bO; };
-  auto load = [&](int q, In& c) {
-    const int od = map_index1(q, A.nd, A.bc) * A.sd;
-    c.rO = __ldg(rho + od + offO); c.mO = __ldg(md + od + offO);
-    if (halo) { c.rX = __ldg(rho + od + offX); c.mX = __ldg(md + od + offX); }
-    else { c.rX = c.rO; c.mX = c.mO; }
-    if (exR) { c.rE = __ldg(rho + od + offR); c.mE = __ldg(md + od + offR); }
-    if (exC) { c.rF = __ldg(rho + od + offC); c.mF = __ldg(md + od + offC); }
-    c.bX = __ldg(A.bx + od + offX);
-    c.bO = __ldg(A.bo + od + offO);
+  struct In { real rO, mO, rX, mX, bX, bO, bD; };
+  In cur, nxt;
+  cur.rX = cur.mX = real(1);
+  cur.bX = cur.bD = real(0);
+  nxt = cur;
+  int qn = n0 - 4;                                                    // next cell to load
+  int off = (n0 - 8) * A.sd + offO;                                   // output cell m = q - 4 = n0 + it - 8
+  // loads of march step `it+1` (cell qn) and B_d of the cell that step finishes, issued one step ahead
+  auto load = [&](In& c, int it_next) {
+    const int od = map_index1(qn, A.nd, A.bc) * A.sd;                 // index mapped by the boundary rule (reading R9)
+    const int iO = od + offO;
+    c.rO = __ldg(rho + iO); c.mO = __ldg(md + iO); c.bO = __ldg(bop + iO);
+    if (halo) {
+      if (xload) { const int iXx = od + offX; c.rX = __ldg(rho + iXx); c.mX = __ldg(md + iXx); c.bX = __ldg(bxp + iXx); }
+    } else {
+      c.bX = __ldg(bxp + iO);
+      if (ROLE == 1) { const int iR = od + offX; c.rX = __ldg(rho + iR); c.mX = __ldg(md + iR); }
+      const int mn = n0 + it_next - 8;
+      if (it_next >= 8 && mn < n1) c.bD = __ldg(bdp + (off + A.sd));
+    }
+    ++qn;
   };
 
-  BPipe<real> px, po;
+  BPipe4<real> px, po;
   px.init(); po.init();
-  In cur, nxt;
-  cur.rE = cur.mE = cur.rF = cur.mF = real(1);
-  nxt = cur;
-  load(n0 - 4, cur);
-  for (int q = n0 - 4; q < n1 + 4; ++q) {
-    const int buf = q & 1;
-    const int m = q - 4;
-    real bdv = real(0);
-    if (!halo && m >= n0) bdv = __ldg(A.bd + m * A.sd + offO);
-    if (q + 1 < n1 + 4) load(q + 1, nxt);
+  load(cur, 0);
+  const int niter = n1 - n0 + 8;                                      // cells n0-4 .. n1+3
+
+  auto step = [&](auto Ktag, int it) {
+    constexpr int K = decltype(Ktag)::value;
+    real* buf = sm + (K & 1) * T::BUF;
+    load(nxt, it + 1);
     // publish rho, m_d of this march step and the fluxes finished in the previous one
-    sR[buf][tO] = cur.rO; sM[buf][tO] = cur.mO;
-    if (halo && hasX) { sR[buf][tX] = cur.rX; sM[buf][tX] = cur.mX; }
-    if (exR) { sR[buf][tR] = cur.rE; sM[buf][tR] = cur.mE; }
-    if (exC) { sR[buf][tC] = cur.rF; sM[buf][tC] = cur.mF; }
-    sFX[buf][fXw] = px.fhi();
-    sFO[buf][fOw] = po.fhi();
-    __syncthreads();
+    buf[tO] = cur.rO; buf[T::NU + tO] = cur.mO;
+    if (halo) { if (xload) { buf[tX] = cur.rX; buf[T::NU + tX] = cur.mX; } }
+    else if (ROLE == 1) { buf[tX] = cur.rX; buf[T::NU + tX] = cur.mX; }
+    buf[fXw] = px.fhi();
+    buf[fOw] = po.fhi();
+    asm volatile("bar.sync 0;" ::: "memory");
     // Alg. 2 step 4: face velocity = momentum sum / density sum of the two cells sharing the face (reading R5)
-    const real vtX = (sM[buf][nbX] + cur.mX) * rcp_(sR[buf][nbX] + cur.rX);
-    const real vtO = (sM[buf][nbO] + cur.mO) * rcp_(sR[buf][nbO] + cur.rO);
-    px.push(vtX, cur.bX, dt, hdt);
-    po.push(vtO, cur.bO, dt, hdt);
-    if (!halo && m >= n0) {
-      const int off = m * A.sd + offO;
-      A.bxo[off] = px.bold() - (px.fhi() - px.flo());        // Alg. 2 step 9: advect B_t
-      A.boo[off] = po.bold() - (po.fhi() - po.flo());
-      // constraint with the same fluxes at face m-1/2: the neighbours published theirs above
-      const real cx = sFX[buf][fXr] - px.flo();
-      const real co = sFO[buf][fOr] - po.flo();
-      const bool x_first = (A.x_is_t1 != 0) != (A.t2_first != 0);   // forward: t1 then t2; reverse: t2 then t1
-      if (x_first) { bdv = bdv + cx; bdv = bdv + co; }
-      else         { bdv = bdv + co; bdv = bdv + cx; }
-      A.bdo[off] = bdv;
+    const real rXc = halo ? cur.rX : cur.rO, mXc = halo ? cur.mX : cur.mO;
+    const real vtX = (buf[T::NU + nbX] + mXc) * rcp_(buf[nbX] + rXc);
+    const real vtO = (buf[T::NU + nbO] + cur.mO) * rcp_(buf[nbO] + cur.rO);
+    real bxn, bon, fxlo, folo;
+    px.template push<K>(vtX, cur.bX, dt, hdt, bxn, fxlo);
+    po.template push<K>(vtO, cur.bO, dt, hdt, bon, folo);
+    if (!halo) {
+      const int m = n0 + it - 8;
+      if (it >= 8 && m < n1) {
+        A.bxo[off] = bxn;                                             // Alg. 2 step 9: advected B_t
+        A.boo[off] = bon;
+        // constraint with the same fluxes at face m-1/2: the neighbours published theirs above
+        const real cx = buf[fXr] - fxlo;
+        const real co = buf[fOr] - folo;
+        real bdv = cur.bD;
+        if (x_first) { bdv = bdv + cx; bdv = bdv + co; }
+        else         { bdv = bdv + co; bdv = bdv + cx; }
+        A.bdo[off] = bdv;
+      }
     }
+    off += A.sd;
     cur = nxt;
+  };
+  for (int it = 0; it < niter; it += 4) {
+    step(std::integral_constant<int, 0>{}, it);
+    step(std::integral_constant<int, 1>{}, it + 1);
+    step(std::integral_constant<int, 2>{}, it + 2);
+    step(std::integral_constant<int, 3>{}, it + 3);
   }
+}
+
+template <class real, int TX, int TO>
+__global__ void __launch_bounds__((TO + 1) * TX, (TO + 1) * TX <= 320 ? MHD_BTILE_MINB : 1) bpair_tile_kernel(const YZArgs<real> A) {
+  static_assert(2 * TO <= TX && TX % 32 == 0, "tile shape");
+  using T = BTile<real, TX, TO>;
+  __shared__ real sm[2 * T::BUF];
+  const int tid = threadIdx.x;
+  const int row = tid / TX, col = tid - row * TX;
+  if (row == TO) bpair_tile_march<real, TX, TO, 2>(A, sm, row, col);
+  else if (row == 0) bpair_tile_march<real, TX, TO, 1>(A, sm, row, col);
+  else bpair_tile_march<real, TX, TO, 0>(A, sm, row, col);
 }
 
 }  // namespace mhd

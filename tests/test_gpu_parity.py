@@ -339,9 +339,32 @@ def test_b_pair_tile_shapes(B, btile, bc, prec):
             for t in ((t2, t1) if rev else (t1, t2)):
                 oracle.badvect(ref, gamma, bc, d, t, dt)
             for seg in (0, 9):
-                s = _solver(B, f0, gamma, bc, prec, btile=btile, segment=seg)
+                s = _solver(B, f0, gamma, bc, prec, btile=btile, btma=0, segment=seg)
                 s.apply(B.MHD_OP_BPAIR, d, rev, dt)
                 got = s.get_state()
                 s.close()
                 e = max_rel(got, ref)
                 assert worst(e) <= tol, (btile, bc, prec, d, rev, seg, e)
+
+
+@pytest.mark.parametrize("btma,stages", [(1, 4), (1, 6), (1, 8), (2, 6), (3, 6), (4, 6)])
+@pytest.mark.parametrize("bc", [P, O])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_b_pair_tma_tile_march(B, btma, stages, bc, prec):
+    """every tile shape / ring depth of the TMA-fed tile-march B kernel (mhd_btma.cuh), whole pencils and ragged segments"""
+    f0 = random_state(128, 16, 24, seed=91 + bc)
+    gamma, dt = 5.0 / 3.0, 0.19
+    tol = TOL64 if prec == "f64" else TOL32_STEP
+    for d in (1, 2):
+        for rev in (0, 1):
+            ref = _ref_input(f0, prec)
+            t1, t2 = (d + 1) % 3, (d + 2) % 3
+            for t in ((t2, t1) if rev else (t1, t2)):
+                oracle.badvect(ref, gamma, bc, d, t, dt)
+            for seg in (0, 9):
+                s = _solver(B, f0, gamma, bc, prec, btma=btma, bstages=stages, segment=seg)
+                s.apply(B.MHD_OP_BPAIR, d, rev, dt)
+                got = s.get_state()
+                s.close()
+                e = max_rel(got, ref)
+                assert worst(e) <= tol, (btma, stages, bc, prec, d, rev, seg, e)
