@@ -106,7 +106,7 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_path = 0;
   c->opt_btile = 1;
   c->opt_ftma = 8;
-  c->opt_btma = 1;
+  c->opt_btma = 0;
   c->opt_bstages = 6;
   c->sm_count = 148;
   *out = c;
@@ -248,8 +248,23 @@ static bool yz_ok(const mhd_ctx* c, int d) {
   return c->opt_path == 0 && d != 0 && c->n[d] >= 8 && c->n[0] >= 32 && c->N < ((size_t)1 << 31);
 }
 
+// Segment length along the sweep for a march kernel whose blocks cover `pencil_blocks` tiles of the transverse
+// plane: more segments fill the last wave of blocks but every segment re-marches `halo` warm-up cells.
+// Picks the number of segments that minimises  waves * (segment + halo)  for `slots` co-resident blocks.
+static int pick_segment(int nd, long long pencil_blocks, long long slots, int halo) {
+  int best_seg = nd;
+  double best = 1e300;
+  for (int nseg = 1; nseg <= 16 && nd / nseg >= 32; ++nseg) {
+    const int seg = ((nd + nseg - 1) / nseg + 3) & ~3;              // multiple of 4 (the marches are unrolled by 4)
+    const long long blocks = pencil_blocks * ((nd + seg - 1) / seg);
+    const double cost = (double)((blocks + slots - 1) / slots) * (seg + halo);
+    if (cost < best * 0.999) { best = cost; best_seg = seg; }
+  }
+  return best_seg;
+}
+
 template <class real>
-static YZArgs<real> make_yz(mhd_ctx* c, int d) {
+static YZArgs<real> make_yz(mhd_ctx* c, int d, int tile_cells = 128, int blocks_per_sm = 4, int halo = 6) {
   const int o = 3 - d;                        // the other transverse axis (x is always one of them)
   const int stride[3] = {1, c->n[0], c->n[0] * c->n[1]};
   YZArgs<real> A;
@@ -262,10 +277,8 @@ static YZArgs<real> make_yz(mhd_ctx* c, int d) {
   A.dt = &c->sc->dt;
   int seg = c->opt_segment;
   if (seg < 0) {
-    const long long pencils = (long long)A.nx * A.no;
-    const long long want = (long long)c->sm_count * 1024;
-    seg = A.nd;
-    while (seg > 64 && pencils * ((A.nd + seg - 1) / seg) < want) seg = (seg + 1) / 2;
+    const long long pencil_blocks = ((long long)A.nx * A.no + tile_cells - 1) / tile_cells;
+    seg = pick_segment(A.nd, pencil_blocks, (long long)c->sm_count * blocks_per_sm, halo);
   }
   if (seg == 0 || seg > A.nd) seg = A.nd;
   A.seg = seg;
@@ -307,7 +320,7 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
 template <class real>
 static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   const int o = 3 - d;
-  YZArgs<real> A = make_yz<real>(c, d);
+  YZArgs<real> A = make_yz<real>(c, d, 256, 3, 8);
   A.u[0] = (const real*)c->cur[0]; A.u[1] = (const real*)c->cur[1 + d];
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];

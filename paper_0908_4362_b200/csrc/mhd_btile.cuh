@@ -75,6 +75,11 @@ struct BTile {
 // index expressions inside the march loop, every step
 __device__ __forceinline__ void pin_reg(int& v) { asm volatile("" : "+r"(v)); }
 
+#ifndef MHD_BTILE_L2PF
+#define MHD_BTILE_L2PF 4
+#endif
+__device__ __forceinline__ void l2_prefetch(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 #ifndef MHD_BTILE_MINB
 #define MHD_BTILE_MINB 3
 #endif
@@ -142,6 +147,13 @@ __device__ __forceinline__ void bpair_tile_march(const YZArgs<real>& A, real* sm
       if (it_next >= 8 && mn < n1) c.bD = __ldg(bdp + (off + A.sd));
     }
     ++qn;
+#if MHD_BTILE_L2PF > 0
+    {   // the loads above have one march step to arrive; pull the lines of a later step from HBM into L2 now
+      const int ip = map_index1(qn + MHD_BTILE_L2PF - 1, A.nd, A.bc) * A.sd + offO;
+      l2_prefetch(rho + ip); l2_prefetch(md + ip); l2_prefetch(bop + ip);
+      if (!halo) { l2_prefetch(bxp + ip); l2_prefetch(bdp + ip); }
+    }
+#endif
   };
 
   BPipe4<real> px, po;
