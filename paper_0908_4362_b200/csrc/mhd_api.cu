@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <type_traits>
 
 #include "mhd_generic.cuh"
 #include "mhd_yz.cuh"
@@ -14,6 +15,8 @@
 #include "mhd_btile.cuh"
 #include "mhd_yz_tma.cuh"
 #include "mhd_btma.cuh"
+#include "mhd_yz2.cuh"
+#include "mhd_bring.cuh"
 
 using namespace mhd;
 
@@ -42,7 +45,7 @@ struct mhd_ctx {
   long long step_index;
   long long launches;
   // options
-  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages;
+  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages, opt_pack, opt_bring;
   int sm_count;
   char err[512];
 };
@@ -108,6 +111,8 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_ftma = 8;
   c->opt_btma = 0;
   c->opt_bstages = 6;
+  c->opt_pack = 1;
+  c->opt_bring = 1;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -298,8 +303,32 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
-  // TMA bulk-copy ring (mhd_yz_tma.cuh) when rows are whole 16-byte aligned blocks, else register prefetch
   const int D = c->opt_ftma;
+  // fp32: two pencils per thread in packed f2 arithmetic (mhd_yz2.cuh)
+  if constexpr (std::is_same<real, float>::value) {
+    const int P = c->opt_pack == 1 ? (A.nx % 256 == 0 ? 256 : (A.nx % 128 == 0 ? 128 : 0))
+                                   : (c->opt_pack > 1 && A.nx % c->opt_pack == 0 ? c->opt_pack : 0);
+    if (D && P) {
+      const int seg = c->opt_segment >= 0 ? A.seg
+                    : pick_segment(A.nd, ((long long)A.nx / P) * A.no, (long long)c->sm_count * (P == 256 ? 2 : 3), 6);
+      A.seg = seg;
+      const dim3 grid(A.nx / P, A.no, (A.nd + A.seg - 1) / A.seg);
+      void (*k)(const YZArgs<float>) = nullptr;
+      size_t smem = 0;
+#define MHD_P2_CASE(P_)                                                                                       \
+      case P_: smem = FluidRing<float, P_>::smem_bytes(8);                                                    \
+        k = A.x_is_t1 ? fluid_yz_p2_kernel<P_, 8, true> : fluid_yz_p2_kernel<P_, 8, false>; break;
+      switch (P) { MHD_P2_CASE(256) default: MHD_P2_CASE(128) }
+#undef MHD_P2_CASE
+      CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k<<<grid, P / 2 + 32, smem, c->stream>>>(A);
+      c->launches++;
+      CUDA_TRY(c, cudaGetLastError());
+      for (int k2 = 0; k2 < 5; ++k2) { void* t = c->cur[role[k2]]; c->cur[role[k2]] = c->alt[role[k2]]; c->alt[role[k2]] = t; }
+      return MHD_OK;
+    }
+  }
+  // TMA bulk-copy ring (mhd_yz_tma.cuh) when rows are whole 16-byte aligned blocks, else register prefetch
   const int TXB = A.nx % 128 == 0 ? 128 : (A.nx % 32 == 0 ? 32 : 0);
   if (D && TXB && (A.nx * sizeof(real)) % 16 == 0) {
     const dim3 grid(A.nx / TXB, A.no, (A.nd + A.seg - 1) / A.seg);
@@ -325,6 +354,31 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];
   A.t2_first = t2_first;
+  // barrier-free row march fed by a TMA ring, packed f2 arithmetic in fp32 (mhd_bring.cuh)
+  if (c->opt_bring) {
+    using T = typename std::conditional<std::is_same<real, float>::value, f2, real>::type;
+    const int W = c->opt_bring > 1 ? c->opt_bring : (std::is_same<real, float>::value && A.nx % 256 == 0 ? 256 : 128);
+    if (A.nx % W == 0 && (W == 128 || (W == 256 && std::is_same<real, float>::value))) {
+      if (c->opt_segment < 0)
+        A.seg = pick_segment(A.nd, ((long long)A.nx / W) * A.no, (long long)c->sm_count * 2, 8);
+      const dim3 grid(A.nx / W, A.no, (A.nd + A.seg - 1) / A.seg);
+      constexpr int D = 8;
+      void (*k)(const YZArgs<real>) = nullptr;
+      size_t smem = 0;
+      int nthr = 0;
+      if (W == 256) {
+        if constexpr (std::is_same<real, float>::value) {
+          k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); nthr = 256 / PackOf<T>::L + 32;
+        }
+      } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); nthr = 128 / PackOf<T>::L + 32; }
+      CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k<<<grid, nthr, smem, c->stream>>>(A);
+      c->launches++;
+      CUDA_TRY(c, cudaGetLastError());
+      for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+      return MHD_OK;
+    }
+  }
   // TMA-fed tile march (mhd_btma.cuh) when rows are whole 16-byte aligned blocks and the extents tile evenly
   {
     static const int shp[5][2] = {{0, 0}, {32, 8}, {64, 4}, {128, 2}, {64, 8}};
@@ -692,6 +746,8 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   if (!strcmp(key, "btma")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btma must be 0..4"); c->opt_btma = (int)value; return MHD_OK; }
   if (!strcmp(key, "bstages")) { if (value != 4 && value != 6 && value != 8) return fail(c, MHD_EINVAL, "bstages must be 4, 6 or 8"); c->opt_bstages = (int)value; return MHD_OK; }
   if (!strcmp(key, "btile")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btile must be 0..4"); c->opt_btile = (int)value; return MHD_OK; }
+  if (!strcmp(key, "bring")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "bring must be 0, 1, 128 or 256"); c->opt_bring = (int)value; return MHD_OK; }
+  if (!strcmp(key, "pack")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "pack must be 0, 1, 128 or 256"); c->opt_pack = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
   return fail(c, MHD_EINVAL, "unknown option '%s'", key);
 }

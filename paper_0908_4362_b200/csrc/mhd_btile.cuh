@@ -43,16 +43,16 @@ struct BPipe4 {
 
   template <int K>
   __device__ __forceinline__ void push(real vtn, real btn, real dt, real hdt, real& bnew, real& flo) {
-    const real vg1 = real(0.25) * ((vt[K & 1] + vtn) + real(2) * vt[(K + 1) & 1]);   // eq (20) at k-1
+    const real vg1 = real(0.25) * fma_(real(2), vt[(K + 1) & 1], vt[K & 1] + vtn);   // eq (20) at k-1
     const real w01 = vg1 * b[(K + 3) & 3];
     const real vh2 = vg + vg1;                                                       // 2 * eq (22) at face (k-2)+1/2
-    const real f1n = vh2 > real(0) ? w0 : w01;                                       // eq (21)
-    const real bh = b[(K + 2) & 3] - (f1n - f1) * hdt;                               // Alg. 2 step 7: B_t^{t+dt/2}(k-2)
+    const real f1n = pick_pos(vh2, w0, w01);                                         // eq (21)
+    const real bh = fnma_(f1n - f1, hdt, b[(K + 2) & 3]);                            // Alg. 2 step 7: B_t^{t+dt/2}(k-2)
     const real wD = vg * bh;
     // Alg. 2 step 8: second-order TVD flux at face (k-4)+1/2, upwinded by the sign of the face velocity there
-    const bool up = vh[K & 1] > real(0);
+    const real up = vh[K & 1];
     const real wA = w1[(K + 3) & 3], wB = w1[K & 3], wC = w1[(K + 1) & 3];           // at k-5, k-4, k-3
-    const real x = up ? wB : wC, y = up ? wA : wD, z = up ? wC : wB;
+    const real x = pick_pos(up, wB, wC), y = pick_pos(up, wA, wD), z = pick_pos(up, wC, wB);
     const real fn = (x + vl_full(x - y, z - x)) * dt;
     bnew = b[K & 3] - (fn - f);                                                      // Alg. 2 step 9 at cell k-4
     flo = f;

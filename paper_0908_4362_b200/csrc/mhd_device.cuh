@@ -9,6 +9,7 @@
 // (1e-12 tolerance).  No --use_fast_math: the discrete switches (a*b > 0, vh > 0) see IEEE products.
 #pragma once
 #include <cuda_runtime.h>
+#include "mhd_pack.cuh"
 
 namespace mhd {
 
@@ -35,6 +36,20 @@ __device__ __forceinline__ float sqrt_(float x) { float r; asm("sqrt.approx.ftz.
 __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
 __device__ __forceinline__ float abs_(float x) { return fabsf(x); }
 __device__ __forceinline__ double abs_(double x) { return fabs(x); }
+// a*b + c and c - a*b as one rounding (the scalar forms are what nvcc's contraction produces anyway;
+// they are spelled out so that the packed type f2 of mhd_pack.cuh gets FFMA2 in the same places)
+__device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float fnma_(float a, float b, float c) { return fmaf(-a, b, c); }
+__device__ __forceinline__ double fnma_(double a, double b, double c) { return fma(-a, b, c); }
+// the two discrete switches of the scheme (reading R8: strict > 0)
+__device__ __forceinline__ float pos_or_zero(float s, float r) { return s > 0.0f ? r : 0.0f; }
+__device__ __forceinline__ double pos_or_zero(double s, double r) { return s > 0.0 ? r : 0.0; }
+__device__ __forceinline__ float pick_pos(float s, float a, float b) { return s > 0.0f ? a : b; }
+__device__ __forceinline__ double pick_pos(double s, double a, double b) { return s > 0.0 ? a : b; }
+// |v| + sqrt(|t| * inv): the freezing speed of PAPER.md:126 from v, t = gamma p + B^2, inv = 1/rho
+__device__ __forceinline__ float freeze_speed(float v, float t, float inv) { return fabsf(v) + sqrt_(fabsf(t) * inv); }
+__device__ __forceinline__ double freeze_speed(double v, double t, double inv) { return fabs(v) + sqrt_(fabs(t) * inv); }
 
 // van Leer limiter of two HALF differences, eq (14), written for the FULL differences
 // a, b:  vanleer(a/2, b/2) = 2 (a/2)(b/2) / (a/2 + b/2) = a b / (a + b).  Zero unless a*b > 0
@@ -43,7 +58,7 @@ template <class real>
 __device__ __forceinline__ real vl_full(real a, real b) {
   const real ab = a * b;
   const real r = ab * rcp_(a + b);
-  return ab > real(0) ? r : real(0);
+  return pos_or_zero(ab, r);
 }
 
 // Cell-centred field of one cell (held fixed through both stages) and what the two
@@ -54,7 +69,7 @@ struct BCell {
   real hb2;          // |b|^2 / 2
   __device__ __forceinline__ void set(real x, real y, real z) {
     b0 = x; b1 = y; b2 = z;
-    hb2 = real(0.5) * (x * x + y * y + z * z);
+    hb2 = real(0.5) * fma_(x, x, fma_(y, y, z * z));
   }
 };
 
@@ -67,22 +82,21 @@ __device__ __forceinline__ void right_left(const real u[5], const BCell<real>& B
   const real m1 = u[1], m2 = u[2], m3 = u[3], E = u[4];
   const real inv = rcp_(u[0]);
   const real v = m1 * inv;
-  const real ke2 = m1 * m1 + m2 * m2 + m3 * m3;
-  const real p = (gamma - real(1)) * ((E - B.hb2) - real(0.5) * (ke2 * inv));
+  const real ke2 = fma_(m1, m1, fma_(m2, m2, m3 * m3));
+  const real p = (gamma - real(1)) * fnma_(real(0.5) * ke2, inv, E - B.hb2);
   const real ps = p + B.hb2;
-  const real bdotv = (B.b0 * m1 + B.b1 * m2 + B.b2 * m3) * inv;
+  const real bdotv = fma_(B.b0, m1, fma_(B.b1, m2, B.b2 * m3)) * inv;
   real F[5];
   F[0] = m1;
-  F[1] = m1 * v + (ps - B.b0 * B.b0);
-  F[2] = m2 * v - B.b1 * B.b0;
-  F[3] = m3 * v - B.b2 * B.b0;
-  F[4] = (E + ps) * v - B.b0 * bdotv;
-  const real c = abs_(v) + sqrt_(abs_(gamma * p + real(2) * B.hb2) * inv);
+  F[1] = fma_(m1, v, fnma_(B.b0, B.b0, ps));
+  F[2] = fnma_(B.b1, B.b0, m2 * v);
+  F[3] = fnma_(B.b2, B.b0, m3 * v);
+  F[4] = fnma_(B.b0, bdotv, (E + ps) * v);
+  const real c = freeze_speed(v, fma_(gamma, p, real(2) * B.hb2), inv);
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
-    const real cu = c * u[k];
-    R[k] = cu + F[k];
-    G[k] = cu - F[k];
+    R[k] = fma_(c, u[k], F[k]);
+    G[k] = fma_(c, u[k], -F[k]);
   }
 }
 
@@ -120,6 +134,14 @@ __device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
   return v;
 }
 
+// Fold a warp's maximum into the global accumulator.  A million warps hitting one address with atomicMax
+// serialise in L2 (measured: +1.4 ms on fluid_x at 512^3), so the atomic is issued only when the value
+// beats what the accumulator already holds; a stale read merely costs one redundant atomic.  The result
+// is still the exact maximum, independent of order.
+__device__ __forceinline__ void publish_max(unsigned long long* acc, unsigned long long v) {
+  if (v > *reinterpret_cast<volatile unsigned long long*>(acc)) atomicMax(acc, v);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Register pipeline of fluid_d for one pencil, fed one cell per call in sweep order.
 // Algorithm 1: first-order upwind half step eq (16), then the second-order TVD
@@ -154,13 +176,22 @@ struct FluidPipe {
 
   // u, B: cell q.  out: updated u of cell q-3.  hdt = dt/2, qdt = dt/4.
   __device__ __forceinline__ void push(const real u[5], const BCell<real>& B, real gamma, real hdt, real qdt, real out[5]) {
+    advance(u, u1_, u3_, B, gamma, hdt, qdt, out);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) { u3_[k] = u2_[k]; u2_[k] = u1_[k]; u1_[k] = u[k]; }
+  }
+
+  // The same step with u(q-1) and u(q-3) supplied by the caller (kernels that keep the input rows in a
+  // shared-memory ring re-read them there instead of spending 15 registers per pencil on a delay line).
+  __device__ __forceinline__ void advance(const real u[5], const real um1[5], const real um3[5], const BCell<real>& B,
+                                          real gamma, real hdt, real qdt, real out[5]) {
     real R0[5], G0[5];
     right_left(u, B, gamma, R0, G0);                 // Alg. 1 step 4 at cell q
     real uh[5], d1[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
       d1[k] = R0_[k] - G0[k];                        // step 5: 2 * first-order flux at face (q-1)+1/2
-      uh[k] = u1_[k] - (d1[k] - d1_[k]) * qdt;       // step 6: u^{t+dt/2}(q-1), eq (16)
+      uh[k] = fnma_(d1[k] - d1_[k], qdt, um1[k]);    // step 6: u^{t+dt/2}(q-1), eq (16)
     }
     real Rc[5], Gc[5];
     right_left(uh, B1_, gamma, Rc, Gc);              // step 7 at cell q-1 (same B_c)
@@ -173,7 +204,7 @@ struct FluidPipe {
       const real dGb = Gb_[k] - Gc[k];
       const real Gp = Gb_[k] + vl_full(dGb, dGa_[k]);
       const real phi2 = Rp_[k] - Gp;                 // 2 * flux at face (q-3)+1/2
-      out[k] = u3_[k] - (phi2 - phi2_[k]) * hdt;     // step 9, eq (17) at cell q-3
+      out[k] = fnma_(phi2 - phi2_[k], hdt, um3[k]);  // step 9, eq (17) at cell q-3
       // shift the window by one cell
       phi2_[k] = phi2;
       Rp_[k] = Rp;
@@ -181,7 +212,6 @@ struct FluidPipe {
       dGa_[k] = dGb; Gb_[k] = Gc[k];
       d1_[k] = d1[k];
       R0_[k] = R0[k];
-      u3_[k] = u2_[k]; u2_[k] = u1_[k]; u1_[k] = u[k];
     }
     hb2_out_ = hb2_3_;
     hb2_3_ = hb2_2_; hb2_2_ = B1_.hb2;
@@ -211,15 +241,14 @@ struct BPipe {
   }
 
   __device__ __forceinline__ void push(real vt, real bt, real dt, real hdt) {
-    const real vg1 = real(0.25) * ((vt2_ + vt) + real(2) * vt1_);      // eq (20) at q-1
+    const real vg1 = real(0.25) * fma_(real(2), vt1_, vt2_ + vt);      // eq (20) at q-1
     const real w01 = vg1 * b1_;
     const real vh = vg2_ + vg1;                                         // 2 * eq (22) at face (q-2)+1/2
-    const real f1 = vh > real(0) ? w02_ : w01;                          // eq (21)
-    const real bh = b2_ - (f1 - f1_) * hdt;                             // Alg. 2 step 7: B_t^{t+dt/2}(q-2)
+    const real f1 = pick_pos(vh, w02_, w01);                            // eq (21)
+    const real bh = fnma_(f1 - f1_, hdt, b2_);                          // Alg. 2 step 7: B_t^{t+dt/2}(q-2)
     const real wD = vg2_ * bh;
     // Alg. 2 step 8: second-order TVD flux at face (q-4)+1/2, upwinded by the sign of vhA_
-    const bool up = vhA_ > real(0);
-    const real x = up ? wB_ : wC_, y = up ? wA_ : wD, z = up ? wC_ : wB_;
+    const real x = pick_pos(vhA_, wB_, wC_), y = pick_pos(vhA_, wA_, wD), z = pick_pos(vhA_, wC_, wB_);
     const real f = x + vl_full(x - y, z - x);
     flo_ = f_;
     f_ = f * dt;

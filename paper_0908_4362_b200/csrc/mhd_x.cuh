@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(256) fluid_x_kernel(const XArgs<real> A) {
       cbest = b > cbest ? b : cbest;
     }
     cbest = warp_max_u64(live ? cbest : 0ull);
-    if ((tid & 31) == 0) atomicMax(A.cmax_bits, cbest);
+    if ((tid & 31) == 0) publish_max(A.cmax_bits, cbest);
   }
 }
 

@@ -114,7 +114,7 @@ _Pragma(MHD_STR(unroll MHD_YZ_UNROLL))
   }
   if (A.cmax_bits) {
     cbest = warp_max_u64(cbest);
-    if ((threadIdx.x & 31) == 0) atomicMax(A.cmax_bits, cbest);
+    if ((threadIdx.x & 31) == 0) publish_max(A.cmax_bits, cbest);
   }
 }
 

@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(TXB + 32, (TXB == 128 && sizeof(real) == 4) ? 
   }
   if (A.cmax_bits) {
     cbest = warp_max_u64(cbest);
-    if ((tid & 31) == 0) atomicMax(A.cmax_bits, cbest);
+    if ((tid & 31) == 0) publish_max(A.cmax_bits, cbest);
   }
 }
 

@@ -49,7 +49,8 @@ def _ref_input(f, prec):
 
 
 SHAPES = [(40, 24, 20), (48, 1, 1), (1, 40, 1), (1, 1, 36), (32, 20, 1), (1, 24, 16), (20, 1, 24), (7, 5, 3),
-          (136, 9, 8), (520, 3, 2), (64, 33, 1), (64, 16, 16), (32, 8, 24)]
+          (136, 9, 8), (520, 3, 2), (64, 33, 1), (64, 16, 16), (32, 8, 24),
+          (128, 12, 10), (256, 9, 11), (384, 10, 1)]     # nx % 128 == 0: the packed (f2) fp32 kernels
 
 
 @pytest.mark.parametrize("path", [0, 1])          # 0: specialised x / yz kernels where they apply, 1: generic kernels only
@@ -368,3 +369,49 @@ def test_b_pair_tma_tile_march(B, btma, stages, bc, prec):
                 s.close()
                 e = max_rel(got, ref)
                 assert worst(e) <= tol, (btma, stages, bc, prec, d, rev, seg, e)
+
+
+@pytest.mark.parametrize("pack", [0, 1, 128, 256])
+@pytest.mark.parametrize("bc", [P, O])
+def test_packed_fp32_kernels(B, pack, bc):
+    """fp32 kernels that advance two pencils per thread in packed f2 arithmetic (mhd_yz2.cuh, mhd_bring.cuh): every row width
+    they accept, several segments with a ragged tail, the fused c_max reduction, against the scalar path"""
+    nx, ny, nz = 512, 22, 19
+    f0 = random_state(nx, ny, nz, seed=77 + bc)
+    gamma, dt = 5.0 / 3.0, 0.19
+    for seg in (-1, 9):
+        for s0 in range(3):
+            ref = _ref_input(f0, "f32")
+            oracle.step_fixed(ref, gamma, bc, s0, dt)
+            s = _solver(B, f0, gamma, bc, "f32", pack=pack, bring=pack, segment=seg)
+            s.step_index = s0
+            s.step_fixed(1, dt)
+            got = s.get_state()
+            _, cmg = s.cfl_dt(0.8)               # c_max fused into the last fluid kernel of the step
+            s.close()
+            e = max_rel(got, ref)
+            assert worst(e) <= TOL32_STEP, (pack, bc, seg, s0, e)
+            cm = oracle.cmax([np.array(a, dtype=np.float64) for a in got], gamma, bc)
+            assert abs(cmg - cm) <= 2e-6 * cm, (pack, bc, seg, s0, cmg, cm)
+
+
+@pytest.mark.parametrize("bring", [0, 1])
+@pytest.mark.parametrize("bc", [P, O])
+def test_b_pair_ring_march_fp64(B, bring, bc):
+    """the barrier-free B-pair row march (mhd_bring.cuh) in fp64, forward and reverse order, ragged segments"""
+    nx, ny, nz = 256, 13, 21
+    f0 = random_state(nx, ny, nz, seed=91 + bc)
+    gamma, dt = 5.0 / 3.0, 0.23
+    for seg in (-1, 10):
+        for d in (1, 2):
+            for rev in (0, 1):
+                ref = _ref_input(f0, "f64")
+                t1, t2 = (d + 1) % 3, (d + 2) % 3
+                for t in ((t2, t1) if rev else (t1, t2)):
+                    oracle.badvect(ref, gamma, bc, d, t, dt)
+                s = _solver(B, f0, gamma, bc, "f64", bring=bring, segment=seg)
+                s.apply(B.MHD_OP_BPAIR, d, rev, dt)
+                got = s.get_state()
+                s.close()
+                e = max_rel(got, ref)
+                assert worst(e) <= TOL64, (bring, bc, seg, d, rev, e)
