@@ -304,24 +304,32 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
   const int D = c->opt_ftma;
-  // fp32: two pencils per thread in packed f2 arithmetic (mhd_yz2.cuh)
-  if constexpr (std::is_same<real, float>::value) {
-    const int P = c->opt_pack == 1 ? (A.nx % 256 == 0 ? 256 : (A.nx % 128 == 0 ? 128 : 0))
-                                   : (c->opt_pack > 1 && A.nx % c->opt_pack == 0 ? c->opt_pack : 0);
+  // ring march with u(q-1), u(q-3) re-read from the ring: fp32 two pencils per thread in packed f2
+  // arithmetic, fp64 one pencil per thread (mhd_yz2.cuh)
+  {
+    constexpr bool f32 = std::is_same<real, float>::value;
+    using T = typename std::conditional<f32, f2, real>::type;
+    int P = c->opt_pack == 1 ? (f32 && A.nx % 256 == 0 ? 256 : (A.nx % 128 == 0 ? 128 : 0))
+                             : (c->opt_pack > 1 && A.nx % c->opt_pack == 0 ? c->opt_pack : 0);
+    if (!f32 && P == 256) P = 128;
     if (D && P) {
-      const int seg = c->opt_segment >= 0 ? A.seg
-                    : pick_segment(A.nd, ((long long)A.nx / P) * A.no, (long long)c->sm_count * (P == 256 ? 2 : 3), 6);
-      A.seg = seg;
+      if (c->opt_segment < 0)
+        A.seg = pick_segment(A.nd, ((long long)A.nx / P) * A.no, (long long)c->sm_count * MHD_YZ2_MINB * ((f32 && P == 128) ? 2 : 1), 6);
       const dim3 grid(A.nx / P, A.no, (A.nd + A.seg - 1) / A.seg);
-      void (*k)(const YZArgs<float>) = nullptr;
+      void (*k)(const YZArgs<real>) = nullptr;
       size_t smem = 0;
-#define MHD_P2_CASE(P_)                                                                                       \
-      case P_: smem = FluidRing<float, P_>::smem_bytes(8);                                                    \
-        k = A.x_is_t1 ? fluid_yz_p2_kernel<P_, 8, true> : fluid_yz_p2_kernel<P_, 8, false>; break;
-      switch (P) { MHD_P2_CASE(256) default: MHD_P2_CASE(128) }
-#undef MHD_P2_CASE
+      constexpr int DR = MHD_YZ2_STAGES;
+      if (P == 256) {
+        if constexpr (f32) {
+          smem = FluidRing<real, 256>::smem_bytes(DR);
+          k = A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 256, DR, true> : fluid_yz_ring_kernel<real, T, 256, DR, false>;
+        }
+      } else {
+        smem = FluidRing<real, 128>::smem_bytes(DR);
+        k = A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 128, DR, true> : fluid_yz_ring_kernel<real, T, 128, DR, false>;
+      }
       CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k<<<grid, P / 2 + 32, smem, c->stream>>>(A);
+      k<<<grid, P / PackOf<T>::L, smem, c->stream>>>(A);
       c->launches++;
       CUDA_TRY(c, cudaGetLastError());
       for (int k2 = 0; k2 < 5; ++k2) { void* t = c->cur[role[k2]]; c->cur[role[k2]] = c->alt[role[k2]]; c->alt[role[k2]] = t; }
@@ -360,17 +368,17 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
     const int W = c->opt_bring > 1 ? c->opt_bring : (std::is_same<real, float>::value && A.nx % 256 == 0 ? 256 : 128);
     if (A.nx % W == 0 && (W == 128 || (W == 256 && std::is_same<real, float>::value))) {
       if (c->opt_segment < 0)
-        A.seg = pick_segment(A.nd, ((long long)A.nx / W) * A.no, (long long)c->sm_count * 2, 8);
+        A.seg = pick_segment(A.nd, ((long long)A.nx / W) * A.no, (long long)c->sm_count * MHD_BRING_MINB, 8);
       const dim3 grid(A.nx / W, A.no, (A.nd + A.seg - 1) / A.seg);
-      constexpr int D = 8;
+      constexpr int D = MHD_BRING_STAGES;
       void (*k)(const YZArgs<real>) = nullptr;
       size_t smem = 0;
       int nthr = 0;
       if (W == 256) {
         if constexpr (std::is_same<real, float>::value) {
-          k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); nthr = 256 / PackOf<T>::L + 32;
+          k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); nthr = 256 / PackOf<T>::L;
         }
-      } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); nthr = 128 / PackOf<T>::L + 32; }
+      } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); nthr = 128 / PackOf<T>::L; }
       CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       k<<<grid, nthr, smem, c->stream>>>(A);
       c->launches++;

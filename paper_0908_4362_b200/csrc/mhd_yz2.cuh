@@ -1,144 +1,161 @@
-// mhd_yz2.cuh -- fluid_y / fluid_z for fp32 with two pencils per thread in packed f2 arithmetic.
+// mhd_yz2.cuh -- fluid_y / fluid_z march on a TMA ring; fp32 with two pencils per thread in packed f2
+// arithmetic (T = f2), fp64 with one (T = double).
 //
-// Same march and the same TMA bulk-copy ring as fluid_yz_tma_kernel (mhd_yz_tma.cuh): one producer
-// thread brings the 10 input rows of each march step (5 u, B_d at the next face, B_o at o and o+1,
-// B_x and the 16-byte chunk holding B_x at x0+TXB) into a D-stage shared-memory ring with
-// cp.async.bulk, full/empty mbarriers per stage.  What changes is the consumer: a thread owns the
-// two adjacent columns x0+2c, x0+2c+1, reads them with one 8-byte LDS per row, runs ONE
-// FluidPipe<f2> whose FADD2/FMUL2/FFMA2 advance both pencils per issued instruction (mhd_pack.cuh),
-// and writes 8-byte stores.  Per cell that is about half the issue slots of the scalar kernel.
+// Same march as fluid_yz_tma_kernel (mhd_yz_tma.cuh): the 10 input rows of each march step (5 u, B_d at
+// the next face, B_o at o and o+1, B_x and the 16-byte chunk holding B_x at x0+TXB) are brought into a
+// D-stage shared-memory ring with cp.async.bulk, full/empty mbarriers per stage.  What changes:
+//   * a thread owns L adjacent columns (L = 2: one 8-byte LDS per row, ONE FluidPipe<f2> whose
+//     FADD2/FMUL2/FFMA2 advance both pencils per issued instruction, 8-byte stores; mhd_pack.cuh);
+//   * u(q-1) and u(q-3) are re-read from the ring instead of being carried in registers
+//     (FluidPipe::advance), so a stage is released three march steps after it is first consumed;
+//   * there is no producer warp: every warp is a consumer and the warps take turns (march step modulo
+//     the warp count) at issuing the copies of the stage PF steps ahead, one copy per lane.  A
+//     dedicated producer warp costs a fifth of the block's registers for a thread that issues ten
+//     instructions per step, and five-warp blocks leave one scheduler with three warps, which caps
+//     every thread at 168 registers.
 //
-// Requirements (else fluid_yz_tma_kernel / fluid_yz_kernel run): fp32, nx % TXB == 0.
+// Requirements (else fluid_yz_tma_kernel / fluid_yz_kernel run): nx % TXB == 0.
 #pragma once
 #include "mhd_yz_tma.cuh"
+#include "mhd_pack_io.cuh"
 
 namespace mhd {
 
-// Resident blocks per SM the register budget is cut for (TXB = 256, 128).  Measured at 512^3 (ms per
-// launch): 168 registers (256:2 or 128:3, 6-8 consumer warps per SM) 1.28; 214 registers, no spills
-// (256:1) 1.96; 128 registers with spills (256:3) 1.94; 96 registers (256:4) 3.3.  The scalar kernel: 1.60.
-#ifndef MHD_YZ2_MINB256
-#define MHD_YZ2_MINB256 2
+// Resident blocks per SM the register budget is cut for.  Measured at 512^3 fp32 with the earlier
+// producer-warp version (ms per launch): 168 registers 1.28; 214 registers, no spills, 4 consumer
+// warps per SM 1.96; 128 registers with spills 1.94; 96 registers 3.3.  The scalar kernel: 1.60.
+#ifndef MHD_YZ2_MINB
+#define MHD_YZ2_MINB 2
 #endif
-#ifndef MHD_YZ2_MINB128
-#define MHD_YZ2_MINB128 3
+#ifndef MHD_YZ2_STAGES
+#define MHD_YZ2_STAGES 8
+#endif
+// the warp on duty refills a stage that every warp released SLACK+1 steps ago: with no slack the duty
+// warp waits for the slowest warp every step, which couples the warps like a block barrier
+#ifndef MHD_YZ2_SLACK
+#define MHD_YZ2_SLACK 1
 #endif
 
-template <int TXB, int D, bool XT1>
-__global__ void __launch_bounds__(TXB / 2 + 32, TXB == 256 ? MHD_YZ2_MINB256 : MHD_YZ2_MINB128) fluid_yz_p2_kernel(const YZArgs<float> A) {
-  using RG = FluidRing<float, TXB>;
-  constexpr int NC = TXB / 2;                            // consumer threads
+// real: element type in memory.  T: arithmetic pack (f2 for float, double for double).
+// D ring stages, PF = D - 4 - SLACK steps of prefetch.
+template <class real, class T, int TXB, int D, bool XT1>
+__global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_ring_kernel(const YZArgs<real> A) {
+  using RG = FluidRing<real, TXB>;
+  typedef typename PackOf<T>::scalar S;
+  constexpr int L = PackOf<T>::L;
+  constexpr int NT = TXB / L;                            // threads (all consumers)
+  constexpr int NW = NT / 32;                            // warps
+  constexpr int PF = D - 4 - MHD_YZ2_SLACK;              // the stage of step it+PF was released at step it+PF-D+3 = it-1-SLACK
+  static_assert(NW >= 1 && (NW & (NW - 1)) == 0 && PF >= 1, "block shape");
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  float* ring = reinterpret_cast<float*>(smem_raw);
+  real* ring = reinterpret_cast<real*>(smem_raw);
   uint64_t* full = reinterpret_cast<uint64_t*>(ring + D * RG::STAGE);
   uint64_t* empty = full + D;
 
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int x0 = blockIdx.x * TXB;
   const int o = blockIdx.y;
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
   const int niter = n1 - n0 + 6;                         // cells n0-3 .. n1+2
   if (tid == 0) {
-    for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NC); }
+    for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
     mbar_fence_init();
   }
   __syncthreads();
 
-  if (tid >= NC) {
-    // ---------------- producer warp: one thread issues all copies ----------------
-    if (tid == NC) {
-      const int rowbase = x0 + o * A.so;
-      const int op_off = (map_index1(o + 1, A.no, A.bc) - o) * A.so;
-      const int xn = map_index1(x0 + TXB, A.nx, A.bc);   // B_x at x0+TXB lives in this 16-byte chunk
-      const int chunk = (xn / RG::CH) * RG::CH + o * A.so;
-      for (int it = 0; it < niter; ++it) {
-        const int s = it % D;
-        if (it >= D) mbar_wait(&empty[s], ((it / D) & 1) ^ 1);
-        const int q = n0 - 3 + it;
-        const int od = map_index1(q, A.nd, A.bc) * A.sd;
-        const int od1 = map_index1(q + 1, A.nd, A.bc) * A.sd;
-        float* st = ring + s * RG::STAGE;
-        mbar_expect_tx(&full[s], RG::BYTES);
-        constexpr uint32_t RB = TXB * sizeof(float);
-#pragma unroll
-        for (int k = 0; k < 5; ++k) bulk_g2s(st + k * RG::ROW, A.u[k] + od + rowbase, RB, &full[s]);
-        bulk_g2s(st + 5 * RG::ROW, A.bd + od1 + rowbase, RB, &full[s]);
-        bulk_g2s(st + 6 * RG::ROW, A.bo + od + rowbase, RB, &full[s]);
-        bulk_g2s(st + 7 * RG::ROW, A.bo + od + rowbase + op_off, RB, &full[s]);
-        bulk_g2s(st + 8 * RG::ROW, A.bx + od + rowbase, RB, &full[s]);
-        bulk_g2s(st + 9 * RG::ROW, A.bx + od + chunk, 16, &full[s]);
-      }
-    }
-    return;
+  // ---- producer duty: lane c < 10 of the warp on duty issues copy c of a stage -----------------------
+  const real* src = nullptr;                             // source row of my copy at march position 0
+  int dst = 0, qshift = 0;
+  uint32_t nbytes = TXB * sizeof(real);
+  {
+    const int rowbase = x0 + o * A.so;
+    const int op_off = (map_index1(o + 1, A.no, A.bc) - o) * A.so;
+    const int xn = map_index1(x0 + TXB, A.nx, A.bc);     // B_x at x0+TXB lives in this 16-byte chunk
+    if (lane < 5) { src = A.u[lane] + rowbase; dst = lane * RG::ROW; }
+    else if (lane == 5) { src = A.bd + rowbase; dst = 5 * RG::ROW; qshift = 1; }
+    else if (lane == 6) { src = A.bo + rowbase; dst = 6 * RG::ROW; }
+    else if (lane == 7) { src = A.bo + rowbase + op_off; dst = 7 * RG::ROW; }
+    else if (lane == 8) { src = A.bx + rowbase; dst = 8 * RG::ROW; }
+    else if (lane == 9) { src = A.bx + (xn / RG::CH) * RG::CH + o * A.so; dst = 9 * RG::ROW; nbytes = 16; }
   }
+  auto produce = [&](int itp) {                          // called by one whole warp
+    const unsigned s = (unsigned)itp % D;
+    if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
+    if (lane < 10) {
+      const int od = map_index1(n0 - 3 + itp + qshift, A.nd, A.bc) * A.sd;
+      if (lane == 0) mbar_expect_tx(&full[s], RG::BYTES);
+      __syncwarp(0x3ffu);
+      bulk_g2s(ring + s * RG::STAGE + dst, src + od, nbytes, &full[s]);
+    }
+    __syncwarp();
+  };
+  for (int itp = warp; itp < PF && itp < niter; itp += NW) produce(itp);
 
-  // ---------------- consumers: two adjacent pencils each ----------------
-  const int c2 = 2 * tid;
+  // ---- consumers: L adjacent pencils each -------------------------------------------------------------
+  const int c2 = L * tid;
   const int base = x0 + c2 + o * A.so;
-  const float dts = (float)(*A.dt);
-  const f2 hdt(0.5f * dts), qdt(0.25f * dts), gamma(A.gamma);
+  const S dts = (S)(*A.dt);
+  const T hdt(S(0.5) * dts), qdt(S(0.25) * dts), gamma(A.gamma);
   const int xn = map_index1(x0 + TXB, A.nx, A.bc);
-  const int xp_idx = 8 * RG::ROW + (c2 + 2 < TXB ? c2 + 2 : TXB + (xn % RG::CH));   // B_x at column c2+2
+  const int xp_idx = 8 * RG::ROW + (c2 + L < TXB ? c2 + L : TXB + (xn % RG::CH));   // B_x at column c2+L
+  T* tag = nullptr;
 
-  FluidPipe<f2> pipe;
+  FluidPipe<T> pipe;
   pipe.init();
-  f2 bd_lo(__ldg(reinterpret_cast<const float2*>(A.bd + map_index1(n0 - 3, A.nd, A.bc) * A.sd + base)));
+  T bd_lo = ld_pack(A.bd + map_index1(n0 - 3, A.nd, A.bc) * A.sd + base, tag);
   unsigned long long cbest = 0ull;
-  // u(q-1) and u(q-3) are re-read from the ring (stages it-1, it-3) instead of being carried in
-  // registers, so a stage is released three march steps after it was first consumed; during the first
-  // three steps those reads return whatever the ring holds: it only feeds warm-up state that is
-  // flushed before the first stored cell, exactly like the dummy values of FluidPipe::init().
+  // During the first three steps the re-reads of u(q-1), u(q-3) return whatever the ring holds: it only
+  // feeds warm-up state that is flushed before the first stored cell, like the dummy values of
+  // FluidPipe::init().
 #pragma unroll 3
   for (int it = 0; it < niter; ++it) {
+    if (((unsigned)it & (NW - 1)) == (unsigned)warp && it + PF < niter) produce(it + PF);
     const unsigned s = (unsigned)it % D;
-    const float* st = ring + s * RG::STAGE;
-    const float* st1 = ring + ((unsigned)(it + D - 1) % D) * RG::STAGE;
-    const float* st3 = ring + ((unsigned)(it + D - 3) % D) * RG::STAGE;
+    const real* st = ring + s * RG::STAGE;
+    const real* st1 = ring + ((unsigned)(it + D - 1) % D) * RG::STAGE;
+    const real* st3 = ring + ((unsigned)(it + D - 3) % D) * RG::STAGE;
     mbar_wait(&full[s], ((unsigned)it / D) & 1);
-    f2 u[5], um1[5], um3[5];
+    T u[5], um1[5], um3[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
-      u[k] = f2(*reinterpret_cast<const float2*>(st + k * RG::ROW + c2));
-      um1[k] = f2(*reinterpret_cast<const float2*>(st1 + k * RG::ROW + c2));
-      um3[k] = f2(*reinterpret_cast<const float2*>(st3 + k * RG::ROW + c2));
+      u[k] = ld_pack(st + k * RG::ROW + c2, tag);
+      um1[k] = ld_pack(st1 + k * RG::ROW + c2, tag);
+      um3[k] = ld_pack(st3 + k * RG::ROW + c2, tag);
     }
-    const f2 bd_hi(*reinterpret_cast<const float2*>(st + 5 * RG::ROW + c2));
-    const f2 boa(*reinterpret_cast<const float2*>(st + 6 * RG::ROW + c2));
-    const f2 bob(*reinterpret_cast<const float2*>(st + 7 * RG::ROW + c2));
-    const f2 bxa(*reinterpret_cast<const float2*>(st + 8 * RG::ROW + c2));
-    const float bxn = st[xp_idx];
-    if (it >= 3) mbar_arrive(&empty[(unsigned)(it + D - 3) % D]);   // stage it-3 is no longer needed
-    const f2 half(0.5f);
-    const f2 boc = half * (boa + bob);
-    const f2 bxc = half * (bxa + f2(bxa.v.y, bxn));      // eq (19): faces -> centre
-    const f2 bdc = half * (bd_lo + bd_hi);
-    BCell<f2> B;
+    const T bd_hi = ld_pack(st + 5 * RG::ROW + c2, tag);
+    const T boa = ld_pack(st + 6 * RG::ROW + c2, tag);
+    const T bob = ld_pack(st + 7 * RG::ROW + c2, tag);
+    const T bxa = ld_pack(st + 8 * RG::ROW + c2, tag);
+    const S bxn = st[xp_idx];
+    if (it >= 3) {                                       // stage it-3 is no longer needed by this warp
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[(unsigned)(it + D - 3) % D]);
+    }
+    const T half(S(0.5));
+    const T boc = half * (boa + bob);
+    const T bxc = half * (bxa + shift_in_right(bxa, bxn));   // eq (19): faces -> centre
+    const T bdc = half * (bd_lo + bd_hi);
+    BCell<T> B;
     if (XT1) B.set(bdc, bxc, boc);       // sweep z: (t1,t2) = (x,y);  sweep y: (t1,t2) = (z,x)
     else     B.set(bdc, boc, bxc);
     bd_lo = bd_hi;
-    f2 out[5];
+    T out[5];
     pipe.advance(u, um1, um3, B, gamma, hdt, qdt, out);
     const int m = n0 - 6 + it;                           // cell q-3
     if (m >= n0) {
       const int off = m * A.sd + base;
 #pragma unroll
-      for (int k = 0; k < 5; ++k) *reinterpret_cast<float2*>(A.uo[k] + off) = out[k].v;
+      for (int k = 0; k < 5; ++k) st_pack(A.uo[k] + off, out[k]);
       if (A.cmax_bits) {          // last operator of a step: c of eq (18) from the updated cells (B unchanged)
-        const float ua[5] = {out[0].v.x, out[1].v.x, out[2].v.x, out[3].v.x, out[4].v.x};
-        const float ub[5] = {out[0].v.y, out[1].v.y, out[2].v.y, out[3].v.y, out[4].v.y};
-        const float ca = cfl_speed_hb2(ua, pipe.hb2_out().v.x, A.gamma);
-        const float cb = cfl_speed_hb2(ub, pipe.hb2_out().v.y, A.gamma);
-        // NaN must win the maximum (it poisons dt): compare the bit patterns, not the floats
-        const unsigned long long ba = speed_bits(ca), bb = speed_bits(cb);
-        const unsigned long long b = ba > bb ? ba : bb;
+        const unsigned long long b = pack_speed_bits(out, pipe.hb2_out(), A.gamma);
         cbest = b > cbest ? b : cbest;
       }
     }
   }
   if (A.cmax_bits) {
     cbest = warp_max_u64(cbest);
-    if ((tid & 31) == 0) publish_max(A.cmax_bits, cbest);
+    if (lane == 0) publish_max(A.cmax_bits, cbest);
   }
 }
 
