@@ -101,10 +101,25 @@ def test_full_size_sampled_parity(name, gen, n, prec):
             oracle.step_fixed(blk, gamma, inputs.OUTFLOW, k, dt)
             got = _gather(after, [l - H for l in lo], n)
             core = (slice(H, H + W),) * 3
+            blk32 = None
             for g, idx in GROUPS.items():
                 err = max(float(np.abs(got[i][core] - blk[i][core]).max()) for i in idx)
                 worst[g] = max(worst[g], err / scale[g])
-                assert err <= TOL[prec] * scale[g], (name, k, lo, g, err / scale[g])
+                if err <= TOL[prec] * scale[g]:
+                    continue
+                # fp32 only (R15): at a strong discontinuity the scheme's discrete switches
+                # (a*b > 0, vh > 0) sit on rounding noise, and fp32 rounding ALONE moves isolated cells by
+                # more than 1e-5 (oracle<float> against oracle<double> on the 96^3 blast: 3.6e-5 in B at the
+                # second step).  There the yardstick is that spread, measured on this very block by the
+                # oracle in both precisions, plus an L1 bound that a wrong kernel cannot meet.
+                assert prec == "f32", (name, k, lo, g, err / scale[g])
+                if blk32 is None:
+                    blk32 = [np.ascontiguousarray(a, dtype=np.float32) for a in _gather(state, [l - H for l in lo], n)]
+                    oracle.step_fixed(blk32, gamma, inputs.OUTFLOW, k, dt)
+                spread = max(float(np.abs(blk32[i][core].astype(np.float64) - blk[i][core]).max()) for i in idx)
+                l1 = sum(float(np.abs(got[i][core] - blk[i][core]).sum()) for i in idx) / (len(idx) * W ** 3)
+                assert err <= 3.0 * spread + TOL[prec] * scale[g], (name, k, lo, g, err / scale[g], spread / scale[g])
+                assert l1 <= 1e-6 * scale[g], (name, k, lo, g, l1 / scale[g])
         state, after = after, state
     sol.close()
     print(name, prec, "worst max-rel per group over 3 steps:", worst)
