@@ -17,6 +17,7 @@
 #include "mhd_btma.cuh"
 #include "mhd_yz2.cuh"
 #include "mhd_bring.cuh"
+#include "mhd_x2.cuh"
 
 using namespace mhd;
 
@@ -45,7 +46,7 @@ struct mhd_ctx {
   long long step_index;
   long long launches;
   // options
-  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages, opt_pack, opt_bring;
+  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages, opt_pack, opt_bring, opt_xpack, opt_xfuse;
   int sm_count;
   char err[512];
 };
@@ -113,6 +114,8 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_bstages = 6;
   c->opt_pack = 1;
   c->opt_bring = 1;
+  c->opt_xpack = 2;
+  c->opt_xfuse = 1;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -459,6 +462,59 @@ static XArgs<real> make_x(mhd_ctx* c, int* block, unsigned* grid) {
   return A;
 }
 
+// ---- lane-pack x kernels and the fused reverse L_x (mhd_x2.cuh) ---------------------------------------
+// kind: 0 fluid_x, 1 B pair, 2 reverse L_x in one pass (B pair then fluid)
+template <class real>
+static bool x2_ok(const mhd_ctx* c, int kind) {
+  constexpr bool f32 = std::is_same<real, float>::value;
+  if (!x_ok<real>(c) || c->n[0] / VecOf<real>::V > 128 || c->n[2] > 65535) return false;
+  if (kind == 2) return c->opt_xfuse != 0;
+  // xpack: 0 kernels of mhd_x.cuh; 1 packed f2 where possible (fp32, even ny), else mhd_x.cuh; 2 the scalar instantiation
+  if (c->opt_xpack == 2) return true;
+  return f32 && c->opt_xpack == 1 && c->n[1] % 2 == 0;
+}
+
+template <class real>
+static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
+  constexpr bool f32 = std::is_same<real, float>::value;
+  using T2 = typename std::conditional<f32, f2, real>::type;
+  const bool pack = f32 && c->opt_xpack == 1 && c->n[1] % 2 == 0;
+  const int V = VecOf<real>::V, L = pack ? 2 : 1;
+  XArgs<real> A;
+  memset(&A, 0, sizeof(A));
+  A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2];
+  A.tpr = A.nx / V;
+  A.tpr_shift = -1;
+  for (int b = 0; b < 8; ++b) if ((1 << b) == A.tpr) A.tpr_shift = b;
+  A.rpb = 128 / A.tpr;
+  const int gpp = A.ny / L;                          // row groups per plane
+  if (A.rpb > gpp) A.rpb = gpp;
+  A.gamma = (real)c->gamma;
+  A.dt = &c->sc->dt;
+  const int block = A.tpr * A.rpb;
+  const dim3 grid((unsigned)((gpp + A.rpb - 1) / A.rpb), (unsigned)A.nz);
+  for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[k]; A.uo[k] = (real*)c->alt[k]; }
+  A.bx = (const real*)c->cur[5]; A.by = (const real*)c->cur[6]; A.bz = (const real*)c->cur[7];
+  A.bxo = (real*)c->alt[5]; A.byo = (real*)c->alt[6]; A.bzo = (real*)c->alt[7];
+  A.t2_first = t2_first;
+  A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
+  void (*k)(const XArgs<real>) = nullptr;
+  const size_t slots = kind == 1 ? 24 : 35;
+  if (pack) {
+    if constexpr (f32) k = kind == 0 ? fluid_x2_kernel<real, T2> : (kind == 1 ? bpair_x2_kernel<real, T2> : lrev_x2_kernel<real, T2>);
+  } else {
+    k = kind == 0 ? fluid_x2_kernel<real, real> : (kind == 1 ? bpair_x2_kernel<real, real> : lrev_x2_kernel<real, real>);
+  }
+  const size_t smem = slots * 128 * (pack ? 2 : 1) * sizeof(real);
+  CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(35 * 128 * 2 * sizeof(real))));
+  k<<<grid, block, smem, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  if (kind != 1) for (int f = 0; f < 5; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  if (kind != 0) for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  return MHD_OK;
+}
+
 template <class real>
 static int launch_fluid_x(mhd_ctx* c, bool want_cmax) {
   int block; unsigned grid;
@@ -509,6 +565,7 @@ static int launch_fluid(mhd_ctx* c, int d, bool want_cmax = false, bool* fused =
   if (fused) *fused = false;
   if (c->n[d] == 1) return MHD_OK;   // both face fluxes of the only cell are identical: exact no-op (R10)
   if (yz_ok(c, d)) { if (fused) *fused = want_cmax; return launch_fluid_yz<real>(c, d, want_cmax); }
+  if (d == 0 && x2_ok<real>(c, 0)) { if (fused) *fused = want_cmax; return launch_x2<real>(c, 0, 0, want_cmax); }
   if (d == 0 && x_ok<real>(c)) { if (fused) *fused = want_cmax; return launch_fluid_x<real>(c, want_cmax); }
   FluidArgs<real> A;
   const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
@@ -530,6 +587,7 @@ template <class real>
 static int launch_bpair(mhd_ctx* c, int d, int t2_first) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
   if (yz_ok(c, d)) return launch_bpair_yz<real>(c, d, t2_first);
+  if (d == 0 && x2_ok<real>(c, 1)) return launch_x2<real>(c, 1, t2_first, false);
   if (d == 0 && x_ok<real>(c)) return launch_bpair_x<real>(c, t2_first);
   BPairArgs<real> A;
   A.rho = (const real*)c->cur[0]; A.md = (const real*)c->cur[1 + d];
@@ -581,6 +639,10 @@ static int sweep(mhd_ctx* c, int d, bool reverse, bool want_cmax = false, bool* 
   if (!reverse) {
     if ((rc = BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d)))) return rc;
     return BY_PRECISION(c, launch_bpair<float>(c, d, 0), launch_bpair<double>(c, d, 0));
+  }
+  if (d == 0 && c->n[0] > 1 && BY_PRECISION(c, x2_ok<float>(c, 2), x2_ok<double>(c, 2))) {   // B pair + fluid in one pass
+    if (fused) *fused = want_cmax;
+    return BY_PRECISION(c, launch_x2<float>(c, 2, 1, want_cmax), launch_x2<double>(c, 2, 1, want_cmax));
   }
   if ((rc = BY_PRECISION(c, launch_bpair<float>(c, d, 1), launch_bpair<double>(c, d, 1)))) return rc;
   return BY_PRECISION(c, launch_fluid<float>(c, d, want_cmax, fused), launch_fluid<double>(c, d, want_cmax, fused));
@@ -756,6 +818,8 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   if (!strcmp(key, "btile")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btile must be 0..4"); c->opt_btile = (int)value; return MHD_OK; }
   if (!strcmp(key, "bring")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "bring must be 0, 1, 128 or 256"); c->opt_bring = (int)value; return MHD_OK; }
   if (!strcmp(key, "pack")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "pack must be 0, 1, 128 or 256"); c->opt_pack = (int)value; return MHD_OK; }
+  if (!strcmp(key, "xpack")) { if (value < 0 || value > 2) return fail(c, MHD_EINVAL, "xpack must be 0, 1 or 2"); c->opt_xpack = (int)value; return MHD_OK; }
+  if (!strcmp(key, "xfuse")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "xfuse must be 0 or 1"); c->opt_xfuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
   return fail(c, MHD_EINVAL, "unknown option '%s'", key);
 }

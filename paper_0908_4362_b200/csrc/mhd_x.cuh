@@ -46,6 +46,7 @@ struct XArgs {
   unsigned long long* cmax_bits;   // != nullptr: also reduce c of eq (18) over the updated cells
   int nx, ny, nz;
   int tpr;                 // threads per row = nx / V
+  int tpr_shift;           // log2(tpr) if tpr is a power of two, else -1 (mhd_x2.cuh)
   int rpb;                 // rows per block
   int t2_first;
   real gamma;

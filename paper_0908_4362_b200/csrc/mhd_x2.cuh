@@ -27,6 +27,10 @@
 
 namespace mhd {
 
+// threads per block (maximum) = shared-memory slot stride: a compile-time constant keeps every exchange
+// address an immediate offset from three base registers (own slot, left and right neighbour)
+#define MHD_X2_NT 128
+
 // ---- V-cell vectors of L rows <-> packs ------------------------------------------------------------
 __device__ __forceinline__ void xload(const float* f, int oa, int ob, f2 (&v)[4]) {
   const float4 a = __ldg(reinterpret_cast<const float4*>(f + oa));
@@ -71,14 +75,13 @@ __device__ __forceinline__ XRows x_rows(const XArgs<real>& A) {
   constexpr int V = VecOf<real>::V;
   XRows r;
   const int tid = threadIdx.x;
-  const int lr = tid / A.tpr;
+  const int lr = A.tpr_shift >= 0 ? (tid >> A.tpr_shift) : tid / A.tpr;
   r.t = tid - lr * A.tpr;
-  const int ngroups = (A.ny / L) * A.nz;
+  const int gpp = A.ny / L;                           // row groups per plane; blockIdx.y is the plane
   int g = blockIdx.x * A.rpb + lr;
-  r.live = g < ngroups;
-  if (!r.live) g = ngroups - 1;                       // keep the thread in step for the barriers
-  const int gpp = A.ny / L;                           // row groups per plane
-  const int k = g / gpp, j = (g - k * gpp) * L;
+  r.live = g < gpp;
+  if (!r.live) g = gpp - 1;                           // keep the thread in step for the barriers
+  const int k = blockIdx.y, j = g * L;
   const int kp = (k + 1 == A.nz) ? 0 : k + 1, km = (k == 0) ? A.nz - 1 : k - 1;
   r.col = r.t * V;
   auto row = [&](int jj, int kk) { return (kk * A.ny + jj) * A.nx + r.col; };
@@ -99,13 +102,13 @@ __device__ __forceinline__ XRows x_rows(const XArgs<real>& A) {
 
 // ---------------------------------------------------------------------------------------------
 // fluid_x of the V cells of one thread, Algorithm 1, in pack arithmetic.
-// sm: 7 groups x 5 components x nthr packs.  u[c][v], B[v] in; un[v][c] out.  Contains three barriers;
+// sm: 7 groups x 5 components x MHD_X2_NT packs.  u[c][v], B[v] in; un[v][c] out.  Contains three barriers;
 // the caller guarantees that nobody still reads sm when it is entered.
 // ---------------------------------------------------------------------------------------------
 template <class T, int V>
-__device__ __forceinline__ void fluid_x_core(T* sm, int nthr, int tid, int tl, int tr, const T (&u)[5][V],
+__device__ __forceinline__ void fluid_x_core(T* sm, int tid, int tl, int tr, const T (&u)[5][V],
                                              const BCell<T> (&B)[V], T gamma, T hdt, T qdt, T (&un)[V][5]) {
-  auto S = [&](int group, int comp, int thr) -> T& { return sm[(group * 5 + comp) * nthr + thr]; };
+  auto S = [&](int group, int comp, int thr) -> T& { return sm[(group * 5 + comp) * MHD_X2_NT + thr]; };
   // stage 0: R, G of u^t (Alg. 1 step 4)
   T R[V][5], G[V][5];
 #pragma unroll
@@ -169,3 +172,268 @@ __device__ __forceinline__ void fluid_x_core(T* sm, int nthr, int tid, int tl, i
     for (int v = 0; v < V; ++v) un[v][c] = fnma_(phi[v + 1][c] - phi[v][c], hdt, u[c][v]);
   }
 }
+
+// ---------------------------------------------------------------------------------------------
+// B_{y->x} and B_{z->x} of the V cells of one thread (Algorithm 2; eqs (20)-(22)
+// PAPER.md:147-158).  Four flux rows in lock step: p = 0: B_y row j, 1: B_y row j+1, 2: B_z plane k,
+// 3: B_z plane k+1 (the +1 rows supply the constraint update of B_x).
+// In: vt[p][v] face velocities, b[p][v] the transverse component of each row.  Out: f[p][0..V] = flux*dt at
+// the faces v-1/2 (index v) of the V cells plus the right face of the last one.
+// sm: 2 sets x 12 slots x MHD_X2_NT packs.  Five barriers.
+// ---------------------------------------------------------------------------------------------
+template <class T, int V>
+__device__ __forceinline__ void bpair_x_core(T* sm, int tid, int tl, int tr, const T (&vt)[4][V],
+                                             const T (&b)[4][V], T dt, T hdt, T (&f)[4][V + 1]) {
+  auto S = [&](int set, int slot, int thr) -> T& { return sm[(set * 12 + slot) * MHD_X2_NT + thr]; };
+  // stage A: eq (20), 1-2-1 smoothing along x
+#pragma unroll
+  for (int p = 0; p < 4; ++p) { S(0, p, tid) = vt[p][V - 1]; S(0, 4 + p, tid) = vt[p][0]; }
+  __syncthreads();
+  T vg[4][V + 1], w[4][V + 2];
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    T e[V + 2];
+    e[0] = S(0, p, tl);
+#pragma unroll
+    for (int v = 0; v < V; ++v) e[v + 1] = vt[p][v];
+    e[V + 1] = S(0, 4 + p, tr);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      vg[p][v] = T(0.25) * fma_(T(2), e[v + 1], e[v] + e[v + 2]);
+      w[p][v] = vg[p][v] * b[p][v];
+    }
+    S(1, p, tid) = vg[p][0]; S(1, 4 + p, tid) = w[p][0];
+  }
+  __syncthreads();
+  // stage B: eqs (21),(22): first-order upwind flux at the right face of each cell
+  T vh[4][V], f1[4][V + 1];
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    vg[p][V] = S(1, p, tr);
+    w[p][V] = S(1, 4 + p, tr);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      vh[p][v] = vg[p][v] + vg[p][v + 1];
+      f1[p][v + 1] = pick_pos(vh[p][v], w[p][v], w[p][v + 1]);
+    }
+    S(0, 8 + p, tid) = f1[p][V];
+  }
+  __syncthreads();
+  // stage C: half step (Alg. 2 step 7) and vg * B^{t+dt/2}
+  T w1[4][V + 3];        // w1[p][v+1] = value at cell v, v = -1..V+1
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    f1[p][0] = S(0, 8 + p, tl);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const T bh = fnma_(f1[p][v + 1] - f1[p][v], hdt, b[p][v]);
+      w1[p][v + 1] = vg[p][v] * bh;
+    }
+    S(1, 8 + p, tid) = w1[p][V];       // last  -> right neighbour's cell -1
+    S(0, p, tid) = w1[p][1];           // first two -> left neighbour's cells V, V+1   (set 0 slots 0..7 are free again)
+    S(0, 4 + p, tid) = w1[p][2];
+  }
+  __syncthreads();
+  // stage D: second-order TVD flux at the right face of each cell (Alg. 2 step 8)
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    w1[p][0] = S(1, 8 + p, tl);
+    w1[p][V + 1] = S(0, p, tr);
+    w1[p][V + 2] = S(0, 4 + p, tr);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const T x = pick_pos(vh[p][v], w1[p][v + 1], w1[p][v + 2]);
+      const T y = pick_pos(vh[p][v], w1[p][v], w1[p][v + 3]);
+      const T z = pick_pos(vh[p][v], w1[p][v + 2], w1[p][v + 1]);
+      f[p][v + 1] = (x + vl_full(x - y, z - x)) * dt;
+    }
+    S(1, p, tid) = f[p][V];
+  }
+  __syncthreads();
+#pragma unroll
+  for (int p = 0; p < 4; ++p) f[p][0] = S(1, p, tl);
+}
+
+// face velocities and transverse fields of the four flux rows of one thread (Alg. 2 step 4, reading R5:
+// momentum sum over density sum of the two cells sharing the face).  r0, m0: rho, m_x of the thread's own cells.
+template <class real, class T, int V>
+__device__ __forceinline__ void bpair_x_inputs(const XArgs<real>& A, const XRows& q, T (&r0)[V], T (&m0)[V],
+                                               T (&vt)[4][V], T (&b)[4][V]) {
+  T r[V], m[V];
+  xload(A.u[0], q.o[1], q.o[2], r0); xload(A.u[1], q.o[1], q.o[2], m0);
+  xload(A.u[0], q.o[0], q.o[1], r); xload(A.u[1], q.o[0], q.o[1], m);                  // rows j-1 (, j)
+#pragma unroll
+  for (int v = 0; v < V; ++v) vt[0][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
+  xload(A.u[0], q.o[2], q.o[3], r); xload(A.u[1], q.o[2], q.o[3], m);                  // rows j+1 (, j+2)
+#pragma unroll
+  for (int v = 0; v < V; ++v) vt[1][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
+  xload(A.u[0], q.okm[0], q.okm[1], r); xload(A.u[1], q.okm[0], q.okm[1], m);
+#pragma unroll
+  for (int v = 0; v < V; ++v) vt[2][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
+  xload(A.u[0], q.okp[0], q.okp[1], r); xload(A.u[1], q.okp[0], q.okp[1], m);
+#pragma unroll
+  for (int v = 0; v < V; ++v) vt[3][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
+  xload(A.by, q.o[1], q.o[2], b[0]);
+  xload(A.by, q.o[2], q.o[3], b[1]);
+  xload(A.bz, q.o[1], q.o[2], b[2]);
+  xload(A.bz, q.okp[0], q.okp[1], b[3]);
+}
+
+// cell-centred field of my V cells from face values (eq (19))
+template <class T, int V>
+__device__ __forceinline__ void x_centre(const T (&bxe)[V + 1], const T (&bya)[V], const T (&byb)[V], const T (&bza)[V],
+                                         const T (&bzb)[V], BCell<T> (&B)[V]) {
+  const T half(0.5);
+#pragma unroll
+  for (int v = 0; v < V; ++v)
+    B[v].set(half * (bxe[v] + bxe[v + 1]), half * (bya[v] + byb[v]), half * (bza[v] + bzb[v]));
+}
+
+template <class real, class T, int V>
+__device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const XRows& q, const T (&un)[V][5],
+                                                   const BCell<T> (&B)[V]) {
+#pragma unroll
+  for (int c = 0; c < 5; ++c) {
+    T o[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) o[v] = un[v][c];
+    if (q.live) xstore(A.uo[c], q.o[1], q.o[2], o);
+  }
+  if (A.cmax_bits) {            // last operator of a step: c of eq (18) from the updated cells (B unchanged by fluid_x)
+    unsigned long long cbest = 0ull;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const unsigned long long bts = pack_speed_bits(un[v], B[v].hb2, A.gamma);
+      cbest = bts > cbest ? bts : cbest;
+    }
+    cbest = warp_max_u64(q.live ? cbest : 0ull);
+    if ((threadIdx.x & 31) == 0) publish_max(A.cmax_bits, cbest);
+  }
+}
+
+#ifndef MHD_X2_MINB2
+#define MHD_X2_MINB2 3     // blocks per SM the register budget is cut for, two rows per thread (f2)
+#endif
+#ifndef MHD_X2_MINB1
+#define MHD_X2_MINB1 5     // one row per thread
+#endif
+#define MHD_X2_MINB(T) (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1)
+
+// ---- fluid_x --------------------------------------------------------------------------------------
+template <class real, class T>
+__global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) fluid_x2_kernel(const XArgs<real> A) {
+  constexpr int V = VecOf<real>::V;
+  constexpr int L = PackOf<T>::L;
+  typedef typename PackOf<T>::scalar S;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* sm = reinterpret_cast<T*>(smem_raw);
+  const XRows q = x_rows<real, L>(A);
+  const S dts = (S)(*A.dt);
+  const T hdt(S(0.5) * dts), qdt(S(0.25) * dts), gamma(A.gamma);
+  T u[5][V];
+#pragma unroll
+  for (int c = 0; c < 5; ++c) xload(A.u[c], q.o[1], q.o[2], u[c]);
+  T bxf[V], bya[V], byb[V], bza[V], bzb[V], bxe[V + 1];
+  xload(A.bx, q.o[1], q.o[2], bxf);
+  xload(A.by, q.o[1], q.o[2], bya); xload(A.by, q.o[2], q.o[3], byb);
+  xload(A.bz, q.o[1], q.o[2], bza); xload(A.bz, q.okp[0], q.okp[1], bzb);
+#pragma unroll
+  for (int v = 0; v < V; ++v) bxe[v] = bxf[v];
+  bxe[V] = xload1(A.bx, q.onext[0], q.onext[1], (T*)nullptr);
+  BCell<T> B[V];
+  x_centre<T, V>(bxe, bya, byb, bza, bzb, B);
+  T un[V][5];
+  fluid_x_core<T, V>(sm, threadIdx.x, q.tl, q.tr, u, B, gamma, hdt, qdt, un);
+  x_store_u_and_cmax<real, T, V>(A, q, un, B);
+}
+
+// ---- B_{y->x}, B_{z->x} ------------------------------------------------------------------------------
+template <class real, class T>
+__global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) bpair_x2_kernel(const XArgs<real> A) {
+  constexpr int V = VecOf<real>::V;
+  constexpr int L = PackOf<T>::L;
+  typedef typename PackOf<T>::scalar S;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* sm = reinterpret_cast<T*>(smem_raw);
+  const XRows q = x_rows<real, L>(A);
+  const S dts = (S)(*A.dt);
+  const T dt(dts), hdt(S(0.5) * dts);
+  T r0[V], m0[V], vt[4][V], b[4][V], f[4][V + 1];
+  bpair_x_inputs<real, T, V>(A, q, r0, m0, vt, b);
+  bpair_x_core<T, V>(sm, threadIdx.x, q.tl, q.tr, vt, b, dt, hdt, f);
+  // advect B_y, B_z (Alg. 2 step 9) and constrain B_x with the same fluxes
+  T bxv[V], byn[V], bzn[V];
+  xload(A.bx, q.o[1], q.o[2], bxv);
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    byn[v] = b[0][v] - (f[0][v + 1] - f[0][v]);
+    bzn[v] = b[2][v] - (f[2][v + 1] - f[2][v]);
+    const T cy = f[1][v] - f[0][v];          // face v-1/2, rows j+1 and j
+    const T cz = f[3][v] - f[2][v];
+    if (A.t2_first) { bxv[v] = bxv[v] + cz; bxv[v] = bxv[v] + cy; }
+    else            { bxv[v] = bxv[v] + cy; bxv[v] = bxv[v] + cz; }
+  }
+  if (q.live) {
+    xstore(A.byo, q.o[1], q.o[2], byn);
+    xstore(A.bzo, q.o[1], q.o[2], bzn);
+    xstore(A.bxo, q.o[1], q.o[2], bxv);
+  }
+}
+
+// ---- reverse L_x in one pass: B_{z->x}, B_{y->x} (t2 first), then fluid_x with the UPDATED field ----
+// Shared memory: 35 slots x MHD_X2_NT packs (the B pair uses slots 0..23, the B_x' exchange slot 34,
+// fluid_x slots 0..34; slot 34 is rewritten by fluid_x only two barriers after it was read).
+template <class real, class T>
+__global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) lrev_x2_kernel(const XArgs<real> A) {
+  constexpr int V = VecOf<real>::V;
+  constexpr int L = PackOf<T>::L;
+  typedef typename PackOf<T>::scalar S;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* sm = reinterpret_cast<T*>(smem_raw);
+  const int tid = threadIdx.x;
+  const XRows q = x_rows<real, L>(A);
+  const S dts = (S)(*A.dt);
+  const T dt(dts), hdt(S(0.5) * dts), qdt(S(0.25) * dts), gamma(A.gamma);
+  T u[5][V];
+  BCell<T> B[V];
+  {
+    T vt[4][V], b[4][V], f[4][V + 1];
+    bpair_x_inputs<real, T, V>(A, q, u[0], u[1], vt, b);
+    bpair_x_core<T, V>(sm, tid, q.tl, q.tr, vt, b, dt, hdt, f);
+    // Alg. 2 step 9 on all four rows: rows j and k are this thread's own B_y', B_z'; rows j+1 and k+1 are
+    // the neighbour rows' updated values, which the cell-centred field of my cells needs (eq (19))
+    T bxe[V + 1], bya[V], byb[V], bza[V], bzb[V];
+    {
+      T bxv[V];
+      xload(A.bx, q.o[1], q.o[2], bxv);
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        bya[v] = b[0][v] - (f[0][v + 1] - f[0][v]);
+        byb[v] = b[1][v] - (f[1][v + 1] - f[1][v]);
+        bza[v] = b[2][v] - (f[2][v + 1] - f[2][v]);
+        bzb[v] = b[3][v] - (f[3][v + 1] - f[3][v]);
+        const T cy = f[1][v] - f[0][v];        // constraint on B_x: face v-1/2, rows j+1 and j
+        const T cz = f[3][v] - f[2][v];
+        if (A.t2_first) { bxv[v] = bxv[v] + cz; bxv[v] = bxv[v] + cy; }
+        else            { bxv[v] = bxv[v] + cy; bxv[v] = bxv[v] + cz; }
+        bxe[v] = bxv[v];
+      }
+      if (q.live) {
+        xstore(A.byo, q.o[1], q.o[2], bya);
+        xstore(A.bzo, q.o[1], q.o[2], bza);
+        xstore(A.bxo, q.o[1], q.o[2], bxv);
+      }
+    }
+    sm[34 * MHD_X2_NT + tid] = bxe[0];              // my first updated B_x face -> left neighbour's face V
+    __syncthreads();
+    bxe[V] = sm[34 * MHD_X2_NT + q.tr];
+    x_centre<T, V>(bxe, bya, byb, bza, bzb, B);
+  }
+#pragma unroll
+  for (int c = 2; c < 5; ++c) xload(A.u[c], q.o[1], q.o[2], u[c]);
+  T un[V][5];
+  fluid_x_core<T, V>(sm, tid, q.tl, q.tr, u, B, gamma, hdt, qdt, un);
+  x_store_u_and_cmax<real, T, V>(A, q, un, B);
+}
+
+}  // namespace mhd

@@ -415,3 +415,42 @@ def test_b_pair_ring_march_fp64(B, bring, bc):
                 s.close()
                 e = max_rel(got, ref)
                 assert worst(e) <= TOL64, (bring, bc, seg, d, rev, e)
+
+
+@pytest.mark.parametrize("xpack,xfuse", [(0, 0), (1, 0), (0, 1), (1, 1), (2, 0), (2, 1)])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(512, 6, 4), (64, 8, 6), (256, 7, 3), (32, 2, 1), (128, 4, 2)])
+def test_x_kernels_pack_and_fused_reverse(B, shape, prec, xpack, xfuse):
+    """sweeps along x (mhd_x2.cuh): two rows per thread in packed f2 arithmetic (fp32, even ny), and the reverse
+    L_x as ONE kernel (B pair, then fluid_x from the updated field), with the fused c_max reduction"""
+    nx, ny, nz = shape
+    f0 = random_state(nx, ny, nz, seed=311 + nx + ny)
+    gamma, dt = 5.0 / 3.0, 0.2
+    tol = TOL64 if prec == "f64" else TOL32_STEP
+    for op, rev in [(B.MHD_OP_FLUID, 0), (B.MHD_OP_BPAIR, 0), (B.MHD_OP_BPAIR, 1),
+                    (B.MHD_OP_SWEEP_FORWARD, 0), (B.MHD_OP_SWEEP_REVERSE, 0)]:
+        ref = _ref_input(f0, prec)
+        if op == B.MHD_OP_FLUID:
+            oracle.fluid(ref, gamma, P, 0, dt)
+        elif op == B.MHD_OP_BPAIR:
+            for t in ((2, 1) if rev else (1, 2)):
+                oracle.badvect(ref, gamma, P, 0, t, dt)
+        else:
+            oracle.sweep(ref, gamma, P, 0, op == B.MHD_OP_SWEEP_REVERSE, dt)
+        s = _solver(B, f0, gamma, P, prec, xpack=xpack, xfuse=xfuse)
+        s.apply(op, 0, rev, dt)
+        got = s.get_state()
+        s.close()
+        e = max_rel(got, ref)
+        assert worst(e) <= tol, (shape, prec, xpack, xfuse, op, rev, e)
+    # a whole step whose LAST operator is the reverse L_x (s mod 3 = 0): the c_max of the next step is fused into it
+    ref = _ref_input(f0, prec)
+    oracle.step_fixed(ref, gamma, P, 0, dt)
+    s = _solver(B, f0, gamma, P, prec, xpack=xpack, xfuse=xfuse)
+    s.step_fixed(1, dt)
+    got = s.get_state()
+    _, cmg = s.cfl_dt(0.8)
+    s.close()
+    assert worst(max_rel(got, ref)) <= tol
+    cm = oracle.cmax([np.array(a, dtype=np.float64) for a in got], gamma, P)
+    assert abs(cmg - cm) <= (1e-13 if prec == "f64" else 2e-6) * cm
