@@ -31,9 +31,41 @@ __device__ __forceinline__ int map_index1(int q, int n, int bc) {
 }
 
 __device__ __forceinline__ float rcp_(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#ifndef MHD_F64_IEEE_DIV
+// fp64: MUFU.RCP64H seed (about 20 bits) + two Newton steps: relative error a few 1e-16, no slow path and no
+// range check, half the dependent DFMA chain of IEEE division.  The fp64 kernels are bound by the latency of
+// exactly these chains (profiles/r01_c5_step_ncu_full.md), and the 1e-12 per-step tolerance leaves ~10^4 ulp.
+// x = 0 or denormal gives NaN, which only ever reaches a discarded select operand (vl_full with a*b <= 0).
+__device__ __forceinline__ double rcp_(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+#else
 __device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
+#endif
 __device__ __forceinline__ float sqrt_(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#ifndef MHD_F64_IEEE_DIV
+// fp64 square root of x >= 0: MUFU.RSQ64H seed, two coupled Newton (Goldschmidt) steps on g ~ sqrt(x), h ~ 1/(2 sqrt(x))
+// and one residual correction; relative error a few 1e-16.
+__device__ __forceinline__ double sqrt_(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double r = fma(-g, h, 0.5);
+  g = fma(g, r, g); h = fma(h, r, h);
+  r = fma(-g, h, 0.5);
+  g = fma(g, r, g); h = fma(h, r, h);
+  const double d = fma(-g, g, x);
+  g = fma(d, h, g);
+  return x > 0.0 ? g : 0.0;
+}
+#else
 __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+#endif
 __device__ __forceinline__ float abs_(float x) { return fabsf(x); }
 __device__ __forceinline__ double abs_(double x) { return fabs(x); }
 // a*b + c and c - a*b as one rounding (the scalar forms are what nvcc's contraction produces anyway;
