@@ -467,7 +467,7 @@ static XArgs<real> make_x(mhd_ctx* c, int* block, unsigned* grid) {
 template <class real>
 static bool x2_ok(const mhd_ctx* c, int kind) {
   constexpr bool f32 = std::is_same<real, float>::value;
-  if (!x_ok<real>(c) || c->n[0] / VecOf<real>::V > 128 || c->n[2] > 65535) return false;
+  if (!x_ok<real>(c) || c->n[0] / VecOf<real>::V > X2Block<real>::NT || c->n[2] > 65535) return false;
   if (kind == 2) return c->opt_xfuse != 0;
   // xpack: 0 kernels of mhd_x.cuh; 1 packed f2 where possible (fp32, even ny), else mhd_x.cuh; 2 the scalar instantiation
   if (c->opt_xpack == 2) return true;
@@ -485,8 +485,9 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2];
   A.tpr = A.nx / V;
   A.tpr_shift = -1;
-  for (int b = 0; b < 8; ++b) if ((1 << b) == A.tpr) A.tpr_shift = b;
-  A.rpb = 128 / A.tpr;
+  for (int b = 0; b < 9; ++b) if ((1 << b) == A.tpr) A.tpr_shift = b;
+  constexpr int NT = X2Block<real>::NT;
+  A.rpb = NT / A.tpr;
   const int gpp = A.ny / L;                          // row groups per plane
   if (A.rpb > gpp) A.rpb = gpp;
   A.gamma = (real)c->gamma;
@@ -505,8 +506,8 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   } else {
     k = kind == 0 ? fluid_x2_kernel<real, real> : (kind == 1 ? bpair_x2_kernel<real, real> : lrev_x2_kernel<real, real>);
   }
-  const size_t smem = slots * 128 * (pack ? 2 : 1) * sizeof(real);
-  CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(35 * 128 * 2 * sizeof(real))));
+  const size_t smem = slots * NT * (pack ? 2 : 1) * sizeof(real);
+  CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(35 * NT * (f32 ? 2 : 1) * sizeof(real))));
   k<<<grid, block, smem, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());

@@ -29,7 +29,7 @@ namespace mhd {
 
 // threads per block (maximum) = shared-memory slot stride: a compile-time constant keeps every exchange
 // address an immediate offset from three base registers (own slot, left and right neighbour)
-#define MHD_X2_NT 128
+template <class real> struct X2Block { static constexpr int NT = sizeof(real) == 4 ? 128 : 256; };
 
 // ---- V-cell vectors of L rows <-> packs ------------------------------------------------------------
 __device__ __forceinline__ void xload(const float* f, int oa, int ob, f2 (&v)[4]) {
@@ -102,13 +102,13 @@ __device__ __forceinline__ XRows x_rows(const XArgs<real>& A) {
 
 // ---------------------------------------------------------------------------------------------
 // fluid_x of the V cells of one thread, Algorithm 1, in pack arithmetic.
-// sm: 7 groups x 5 components x MHD_X2_NT packs.  u[c][v], B[v] in; un[v][c] out.  Contains three barriers;
+// sm: 7 groups x 5 components x NT packs.  u[c][v], B[v] in; un[v][c] out.  Contains three barriers;
 // the caller guarantees that nobody still reads sm when it is entered.
 // ---------------------------------------------------------------------------------------------
-template <class T, int V>
+template <class T, int V, int NT>
 __device__ __forceinline__ void fluid_x_core(T* sm, int tid, int tl, int tr, const T (&u)[5][V],
                                              const BCell<T> (&B)[V], T gamma, T hdt, T qdt, T (&un)[V][5]) {
-  auto S = [&](int group, int comp, int thr) -> T& { return sm[(group * 5 + comp) * MHD_X2_NT + thr]; };
+  auto S = [&](int group, int comp, int thr) -> T& { return sm[(group * 5 + comp) * NT + thr]; };
   // stage 0: R, G of u^t (Alg. 1 step 4)
   T R[V][5], G[V][5];
 #pragma unroll
@@ -179,12 +179,12 @@ __device__ __forceinline__ void fluid_x_core(T* sm, int tid, int tl, int tr, con
 // 3: B_z plane k+1 (the +1 rows supply the constraint update of B_x).
 // In: vt[p][v] face velocities, b[p][v] the transverse component of each row.  Out: f[p][0..V] = flux*dt at
 // the faces v-1/2 (index v) of the V cells plus the right face of the last one.
-// sm: 2 sets x 12 slots x MHD_X2_NT packs.  Five barriers.
+// sm: 2 sets x 12 slots x NT packs.  Five barriers.
 // ---------------------------------------------------------------------------------------------
-template <class T, int V>
+template <class T, int V, int NT>
 __device__ __forceinline__ void bpair_x_core(T* sm, int tid, int tl, int tr, const T (&vt)[4][V],
                                              const T (&b)[4][V], T dt, T hdt, T (&f)[4][V + 1]) {
-  auto S = [&](int set, int slot, int thr) -> T& { return sm[(set * 12 + slot) * MHD_X2_NT + thr]; };
+  auto S = [&](int set, int slot, int thr) -> T& { return sm[(set * 12 + slot) * NT + thr]; };
   // stage A: eq (20), 1-2-1 smoothing along x
 #pragma unroll
   for (int p = 0; p < 4; ++p) { S(0, p, tid) = vt[p][V - 1]; S(0, 4 + p, tid) = vt[p][0]; }
@@ -317,13 +317,17 @@ __device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const X
 #ifndef MHD_X2_MINB1
 #define MHD_X2_MINB1 5     // one row per thread
 #endif
-#define MHD_X2_MINB(T) (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1)
+#ifndef MHD_X2_MINB64
+#define MHD_X2_MINB64 2    // fp64: 256-thread blocks
+#endif
+#define MHD_X2_MINB(real, T) (sizeof(real) == 8 ? MHD_X2_MINB64 : (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1))
 
 // ---- fluid_x --------------------------------------------------------------------------------------
 template <class real, class T>
-__global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) fluid_x2_kernel(const XArgs<real> A) {
+__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) fluid_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
+  constexpr int NT = X2Block<real>::NT;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
@@ -343,15 +347,16 @@ __global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) fluid_x2_kernel(con
   BCell<T> B[V];
   x_centre<T, V>(bxe, bya, byb, bza, bzb, B);
   T un[V][5];
-  fluid_x_core<T, V>(sm, threadIdx.x, q.tl, q.tr, u, B, gamma, hdt, qdt, un);
+  fluid_x_core<T, V, NT>(sm, threadIdx.x, q.tl, q.tr, u, B, gamma, hdt, qdt, un);
   x_store_u_and_cmax<real, T, V>(A, q, un, B);
 }
 
 // ---- B_{y->x}, B_{z->x} ------------------------------------------------------------------------------
 template <class real, class T>
-__global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) bpair_x2_kernel(const XArgs<real> A) {
+__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) bpair_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
+  constexpr int NT = X2Block<real>::NT;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
@@ -360,7 +365,7 @@ __global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) bpair_x2_kernel(con
   const T dt(dts), hdt(S(0.5) * dts);
   T r0[V], m0[V], vt[4][V], b[4][V], f[4][V + 1];
   bpair_x_inputs<real, T, V>(A, q, r0, m0, vt, b);
-  bpair_x_core<T, V>(sm, threadIdx.x, q.tl, q.tr, vt, b, dt, hdt, f);
+  bpair_x_core<T, V, NT>(sm, threadIdx.x, q.tl, q.tr, vt, b, dt, hdt, f);
   // advect B_y, B_z (Alg. 2 step 9) and constrain B_x with the same fluxes
   T bxv[V], byn[V], bzn[V];
   xload(A.bx, q.o[1], q.o[2], bxv);
@@ -381,12 +386,13 @@ __global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) bpair_x2_kernel(con
 }
 
 // ---- reverse L_x in one pass: B_{z->x}, B_{y->x} (t2 first), then fluid_x with the UPDATED field ----
-// Shared memory: 35 slots x MHD_X2_NT packs (the B pair uses slots 0..23, the B_x' exchange slot 34,
+// Shared memory: 35 slots x NT packs (the B pair uses slots 0..23, the B_x' exchange slot 34,
 // fluid_x slots 0..34; slot 34 is rewritten by fluid_x only two barriers after it was read).
 template <class real, class T>
-__global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) lrev_x2_kernel(const XArgs<real> A) {
+__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) lrev_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
+  constexpr int NT = X2Block<real>::NT;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
@@ -399,7 +405,7 @@ __global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) lrev_x2_kernel(cons
   {
     T vt[4][V], b[4][V], f[4][V + 1];
     bpair_x_inputs<real, T, V>(A, q, u[0], u[1], vt, b);
-    bpair_x_core<T, V>(sm, tid, q.tl, q.tr, vt, b, dt, hdt, f);
+    bpair_x_core<T, V, NT>(sm, tid, q.tl, q.tr, vt, b, dt, hdt, f);
     // Alg. 2 step 9 on all four rows: rows j and k are this thread's own B_y', B_z'; rows j+1 and k+1 are
     // the neighbour rows' updated values, which the cell-centred field of my cells needs (eq (19))
     T bxe[V + 1], bya[V], byb[V], bza[V], bzb[V];
@@ -424,15 +430,15 @@ __global__ void __launch_bounds__(MHD_X2_NT, MHD_X2_MINB(T)) lrev_x2_kernel(cons
         xstore(A.bxo, q.o[1], q.o[2], bxv);
       }
     }
-    sm[34 * MHD_X2_NT + tid] = bxe[0];              // my first updated B_x face -> left neighbour's face V
+    sm[34 * NT + tid] = bxe[0];              // my first updated B_x face -> left neighbour's face V
     __syncthreads();
-    bxe[V] = sm[34 * MHD_X2_NT + q.tr];
+    bxe[V] = sm[34 * NT + q.tr];
     x_centre<T, V>(bxe, bya, byb, bza, bzb, B);
   }
 #pragma unroll
   for (int c = 2; c < 5; ++c) xload(A.u[c], q.o[1], q.o[2], u[c]);
   T un[V][5];
-  fluid_x_core<T, V>(sm, tid, q.tl, q.tr, u, B, gamma, hdt, qdt, un);
+  fluid_x_core<T, V, NT>(sm, tid, q.tl, q.tr, u, B, gamma, hdt, qdt, un);
   x_store_u_and_cmax<real, T, V>(A, q, un, B);
 }
 
