@@ -34,6 +34,9 @@ WORKLOADS = {
 }
 ALGO_WORDS_STEP = 96          # ideal: each of the six L_i reads 8 fields and writes 8
 CFL = 0.8
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
+# captures (profiles/r01_c4_step_ncu_full_c.md, profiles/r01_c5_step_ncu_full_b.md); None where no capture exists
+NCU_TRAFFIC = {("c4", "fluid_yz"): 7.059e9, ("c5", "fluid_yz"): 14.07e9}
 
 
 def peaks():
@@ -162,28 +165,20 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_0908_4362_b200.replicas import Replicas, env_rank
+    rank, local_rank, world = env_rank()
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
 
     import torch
-    import torch.distributed as dist
     from paper_0908_4362_b200 import binding as B      # raises if libmhd.so is missing: no fallback
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local_rank)
     device = f"cuda:{local_rank}"
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device(device))
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    rep = Replicas(backend="nccl", device=device)      # replicas only: barrier + max-over-ranks timing, no data-path collective
+    barrier = rep.barrier
 
     gen, n, prec, desc = WORKLOADS[args.workload]
     N = n ** 3
@@ -218,10 +213,7 @@ def main():
         l1 = sol.launch_count()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop(w0, w1)
-    if world > 1:
-        t = torch.tensor([ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = rep.max_over_ranks(ms)
     t_now = sol.time()        # also surfaces a poisoned state
     value = N * world * args.steps / (ms * 1e-3)
 
@@ -231,7 +223,8 @@ def main():
     if rank == 0 and not args.no_breakdown:
         dtv, _ = sol.cfl_dt(CFL)
         kinds = [("fluid_x", B.MHD_OP_FLUID, 0, 13), ("fluid_y", B.MHD_OP_FLUID, 1, 13), ("fluid_z", B.MHD_OP_FLUID, 2, 13),
-                 ("bpair_x", B.MHD_OP_BPAIR, 0, 8), ("bpair_y", B.MHD_OP_BPAIR, 1, 8), ("bpair_z", B.MHD_OP_BPAIR, 2, 8)]
+                 ("bpair_x", B.MHD_OP_BPAIR, 0, 8), ("bpair_y", B.MHD_OP_BPAIR, 1, 8), ("bpair_z", B.MHD_OP_BPAIR, 2, 8),
+                 ("lrev_x", B.MHD_OP_SWEEP_REVERSE, 0, 16)]   # reverse L_x: one fused kernel (fp32) or B pair + fluid
         breakdown = {}
         reps = 5
         with torch.cuda.stream(stream):
@@ -255,12 +248,24 @@ def main():
             torch.cuda.synchronize()
             kms = a.elapsed_time(b) / reps
             breakdown["cfl"] = {"ms": kms, "algo_GBps": 8 * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": 8}
-        # dominant kernel = the fluid kernel with the largest share of a step (each runs twice per step)
-        dom = max(("fluid_x", "fluid_y", "fluid_z"), key=lambda k: breakdown[k]["ms"])
-        ach = breakdown[dom]["algo_GBps"]
+        # Dominant kernel = largest share of a step.  Launches per step, averaged over the three sweep orders:
+        # fluid_y, fluid_z 2 each (one kernel template, fluid_yz_ring_kernel, 4 launches), B pair y/z 2 each
+        # (bpair_ring_kernel, 4 launches), fluid_x 1 + bpair_x 1 (forward L_x) and the reverse L_x (1).
+        share = {"fluid_yz": 2 * (breakdown["fluid_y"]["ms"] + breakdown["fluid_z"]["ms"]),
+                 "bpair_yz": 2 * (breakdown["bpair_y"]["ms"] + breakdown["bpair_z"]["ms"]),
+                 "fluid_x": breakdown["fluid_x"]["ms"], "bpair_x": breakdown["bpair_x"]["ms"],
+                 "lrev_x": breakdown["lrev_x"]["ms"]}
+        dom = max(share, key=share.get)
+        if dom.endswith("_yz"):
+            a_, b_ = breakdown[dom[:-2] + "y"], breakdown[dom[:-2] + "z"]
+            kms, words = 0.5 * (a_["ms"] + b_["ms"]), a_["words_per_cell"]
+        else:
+            kms, words = breakdown[dom]["ms"], breakdown[dom]["words_per_cell"]
+        ach = words * esize * N / (kms * 1e-3) / 1e9
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": None, "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": 13 * esize * N,
+                    "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": words * esize * N, "ms_per_launch": kms,
+                    "share_of_step": share[dom] / sum(share.values()),
                     "step": {"algorithmic_bytes_per_cell_step": ALGO_WORDS_STEP * esize,
                              "achieved": ALGO_WORDS_STEP * esize * (value / world) / 1e9,
                              "frac": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / peak}}
@@ -281,10 +286,7 @@ def main():
             sol.get_state(host)                    # D2H of the step's result
         barrier()
         el = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([el], device=device, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
+        el = rep.max_over_ranks(el)
         e2e = {"value": N * world * k_e2e / el, "unit": "cell-updates/s", "h2d_bytes_per_step": 8 * N * esize,
                "d2h_bytes_per_step": 8 * N * esize, "steps": k_e2e}
         del host
@@ -308,8 +310,7 @@ def main():
         }
         print(json.dumps(out))
     sol.close()
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 if __name__ == "__main__":

@@ -114,7 +114,7 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_bstages = 6;
   c->opt_pack = 1;
   c->opt_bring = 1;
-  c->opt_xpack = 2;
+  c->opt_xpack = 3;
   c->opt_xfuse = 1;
   c->sm_count = 148;
   *out = c;
@@ -468,9 +468,10 @@ template <class real>
 static bool x2_ok(const mhd_ctx* c, int kind) {
   constexpr bool f32 = std::is_same<real, float>::value;
   if (!x_ok<real>(c) || c->n[0] / VecOf<real>::V > X2Block<real>::NT || c->n[2] > 65535) return false;
-  if (kind == 2) return c->opt_xfuse != 0;
-  // xpack: 0 kernels of mhd_x.cuh; 1 packed f2 where possible (fp32, even ny), else mhd_x.cuh; 2 the scalar instantiation
-  if (c->opt_xpack == 2) return true;
+  if (kind == 2) return c->opt_xfuse == 2 || ((c->opt_xfuse == 1 || c->opt_xfuse == 3) && f32);   // fp64: the fused kernel is slower than the pair (profiles/)
+  // xpack: 0 kernels of mhd_x.cuh; 1 packed f2 where possible (fp32, even ny), else mhd_x.cuh; 2 the scalar instantiation;
+  // 3 packed fluid_x (where possible), scalar B pair
+  if (c->opt_xpack >= 2) return true;
   return f32 && c->opt_xpack == 1 && c->n[1] % 2 == 0;
 }
 
@@ -478,7 +479,9 @@ template <class real>
 static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   constexpr bool f32 = std::is_same<real, float>::value;
   using T2 = typename std::conditional<f32, f2, real>::type;
-  const bool pack = f32 && c->opt_xpack == 1 && c->n[1] % 2 == 0;
+  // xfuse = 3: the fused operator in packed f2 arithmetic even when the single operators run scalar
+  // xpack = 3: fluid_x packed (1.23 ms at 512^3, scalar 1.29), B pair scalar (0.89 ms, packed 1.14)
+  const bool pack = f32 && c->n[1] % 2 == 0 && (c->opt_xpack == 1 || (c->opt_xpack == 3 && kind == 0) || (kind == 2 && c->opt_xfuse == 3));
   const int V = VecOf<real>::V, L = pack ? 2 : 1;
   XArgs<real> A;
   memset(&A, 0, sizeof(A));
@@ -487,6 +490,7 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   A.tpr_shift = -1;
   for (int b = 0; b < 9; ++b) if ((1 << b) == A.tpr) A.tpr_shift = b;
   constexpr int NT = X2Block<real>::NT;
+  A.one = (real)1;
   A.rpb = NT / A.tpr;
   const int gpp = A.ny / L;                          // row groups per plane
   if (A.rpb > gpp) A.rpb = gpp;
@@ -819,8 +823,8 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   if (!strcmp(key, "btile")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btile must be 0..4"); c->opt_btile = (int)value; return MHD_OK; }
   if (!strcmp(key, "bring")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "bring must be 0, 1, 128 or 256"); c->opt_bring = (int)value; return MHD_OK; }
   if (!strcmp(key, "pack")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "pack must be 0, 1, 128 or 256"); c->opt_pack = (int)value; return MHD_OK; }
-  if (!strcmp(key, "xpack")) { if (value < 0 || value > 2) return fail(c, MHD_EINVAL, "xpack must be 0, 1 or 2"); c->opt_xpack = (int)value; return MHD_OK; }
-  if (!strcmp(key, "xfuse")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "xfuse must be 0 or 1"); c->opt_xfuse = (int)value; return MHD_OK; }
+  if (!strcmp(key, "xpack")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 0..3"); c->opt_xpack = (int)value; return MHD_OK; }
+  if (!strcmp(key, "xfuse")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xfuse must be 0, 1 (fp32 only), 2 (always) or 3 (fp32, packed)"); c->opt_xfuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
   return fail(c, MHD_EINVAL, "unknown option '%s'", key);
 }

@@ -50,6 +50,7 @@ struct XArgs {
   int rpb;                 // rows per block
   int t2_first;
   real gamma;
+  real one;                // 1.0 at run time (mhd_x2.cuh, xload)
 };
 
 // fluid_x, Algorithm 1.  Shared memory: 7 groups x 5 components x blockDim.x reals.

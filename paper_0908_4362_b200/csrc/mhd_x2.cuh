@@ -32,16 +32,22 @@ namespace mhd {
 template <class real> struct X2Block { static constexpr int NT = sizeof(real) == 4 ? 128 : 256; };
 
 // ---- V-cell vectors of L rows <-> packs ------------------------------------------------------------
-__device__ __forceinline__ void xload(const float* f, int oa, int ob, f2 (&v)[4]) {
+// f2: the two rows arrive as two 16-byte vectors, and a pack must sit in an aligned register PAIR.  ptxas
+// re-forms such a pair with two MOVs at EVERY use of a value that came straight out of a vector load (46 MOVs
+// per cell in a first version of fluid_x, profiles/r01_x2_packing.md).  A value produced by a scalar
+// instruction, however, is allocated directly into its half of the pair, so each loaded value is passed
+// through ONE exact scalar multiplication by a run-time 1.0f (XArgs::one; a literal would be folded away).
+__device__ __forceinline__ void xload(const float* f, int oa, int ob, f2 (&v)[4], float one) {
   const float4 a = __ldg(reinterpret_cast<const float4*>(f + oa));
   const float4 b = __ldg(reinterpret_cast<const float4*>(f + ob));
-  v[0] = f2(a.x, b.x); v[1] = f2(a.y, b.y); v[2] = f2(a.z, b.z); v[3] = f2(a.w, b.w);
+  v[0] = f2(a.x * one, b.x * one); v[1] = f2(a.y * one, b.y * one);
+  v[2] = f2(a.z * one, b.z * one); v[3] = f2(a.w * one, b.w * one);
 }
-__device__ __forceinline__ void xload(const double* f, int oa, int, double (&v)[2]) {
+__device__ __forceinline__ void xload(const double* f, int oa, int, double (&v)[2], double) {
   const double2 a = __ldg(reinterpret_cast<const double2*>(f + oa));
   v[0] = a.x; v[1] = a.y;
 }
-__device__ __forceinline__ void xload(const float* f, int oa, int, float (&v)[4]) {
+__device__ __forceinline__ void xload(const float* f, int oa, int, float (&v)[4], float) {
   const float4 a = __ldg(reinterpret_cast<const float4*>(f + oa));
   v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
 }
@@ -56,7 +62,7 @@ __device__ __forceinline__ void xstore(float* f, int oa, int, const float (&v)[4
   *reinterpret_cast<float4*>(f + oa) = make_float4(v[0], v[1], v[2], v[3]);
 }
 // one element per row
-__device__ __forceinline__ f2 xload1(const float* f, int oa, int ob, f2*) { return f2(__ldg(f + oa), __ldg(f + ob)); }
+__device__ __forceinline__ f2 xload1(const float* f, int oa, int ob, f2*) { return f2(__ldg(f + oa), __ldg(f + ob)); }   // scalar loads land in place
 __device__ __forceinline__ double xload1(const double* f, int oa, int, double*) { return __ldg(f + oa); }
 __device__ __forceinline__ float xload1(const float* f, int oa, int, float*) { return __ldg(f + oa); }
 
@@ -260,23 +266,23 @@ template <class real, class T, int V>
 __device__ __forceinline__ void bpair_x_inputs(const XArgs<real>& A, const XRows& q, T (&r0)[V], T (&m0)[V],
                                                T (&vt)[4][V], T (&b)[4][V]) {
   T r[V], m[V];
-  xload(A.u[0], q.o[1], q.o[2], r0); xload(A.u[1], q.o[1], q.o[2], m0);
-  xload(A.u[0], q.o[0], q.o[1], r); xload(A.u[1], q.o[0], q.o[1], m);                  // rows j-1 (, j)
+  xload(A.u[0], q.o[1], q.o[2], r0, A.one); xload(A.u[1], q.o[1], q.o[2], m0, A.one);
+  xload(A.u[0], q.o[0], q.o[1], r, A.one); xload(A.u[1], q.o[0], q.o[1], m, A.one);                  // rows j-1 (, j)
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[0][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
-  xload(A.u[0], q.o[2], q.o[3], r); xload(A.u[1], q.o[2], q.o[3], m);                  // rows j+1 (, j+2)
+  xload(A.u[0], q.o[2], q.o[3], r, A.one); xload(A.u[1], q.o[2], q.o[3], m, A.one);                  // rows j+1 (, j+2)
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[1][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
-  xload(A.u[0], q.okm[0], q.okm[1], r); xload(A.u[1], q.okm[0], q.okm[1], m);
+  xload(A.u[0], q.okm[0], q.okm[1], r, A.one); xload(A.u[1], q.okm[0], q.okm[1], m, A.one);
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[2][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
-  xload(A.u[0], q.okp[0], q.okp[1], r); xload(A.u[1], q.okp[0], q.okp[1], m);
+  xload(A.u[0], q.okp[0], q.okp[1], r, A.one); xload(A.u[1], q.okp[0], q.okp[1], m, A.one);
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[3][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
-  xload(A.by, q.o[1], q.o[2], b[0]);
-  xload(A.by, q.o[2], q.o[3], b[1]);
-  xload(A.bz, q.o[1], q.o[2], b[2]);
-  xload(A.bz, q.okp[0], q.okp[1], b[3]);
+  xload(A.by, q.o[1], q.o[2], b[0], A.one);
+  xload(A.by, q.o[2], q.o[3], b[1], A.one);
+  xload(A.bz, q.o[1], q.o[2], b[2], A.one);
+  xload(A.bz, q.okp[0], q.okp[1], b[3], A.one);
 }
 
 // cell-centred field of my V cells from face values (eq (19))
@@ -336,11 +342,11 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) fluid
   const T hdt(S(0.5) * dts), qdt(S(0.25) * dts), gamma(A.gamma);
   T u[5][V];
 #pragma unroll
-  for (int c = 0; c < 5; ++c) xload(A.u[c], q.o[1], q.o[2], u[c]);
+  for (int c = 0; c < 5; ++c) xload(A.u[c], q.o[1], q.o[2], u[c], A.one);
   T bxf[V], bya[V], byb[V], bza[V], bzb[V], bxe[V + 1];
-  xload(A.bx, q.o[1], q.o[2], bxf);
-  xload(A.by, q.o[1], q.o[2], bya); xload(A.by, q.o[2], q.o[3], byb);
-  xload(A.bz, q.o[1], q.o[2], bza); xload(A.bz, q.okp[0], q.okp[1], bzb);
+  xload(A.bx, q.o[1], q.o[2], bxf, A.one);
+  xload(A.by, q.o[1], q.o[2], bya, A.one); xload(A.by, q.o[2], q.o[3], byb, A.one);
+  xload(A.bz, q.o[1], q.o[2], bza, A.one); xload(A.bz, q.okp[0], q.okp[1], bzb, A.one);
 #pragma unroll
   for (int v = 0; v < V; ++v) bxe[v] = bxf[v];
   bxe[V] = xload1(A.bx, q.onext[0], q.onext[1], (T*)nullptr);
@@ -368,7 +374,7 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) bpair
   bpair_x_core<T, V, NT>(sm, threadIdx.x, q.tl, q.tr, vt, b, dt, hdt, f);
   // advect B_y, B_z (Alg. 2 step 9) and constrain B_x with the same fluxes
   T bxv[V], byn[V], bzn[V];
-  xload(A.bx, q.o[1], q.o[2], bxv);
+  xload(A.bx, q.o[1], q.o[2], bxv, A.one);
 #pragma unroll
   for (int v = 0; v < V; ++v) {
     byn[v] = b[0][v] - (f[0][v + 1] - f[0][v]);
@@ -411,7 +417,7 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) lrev_
     T bxe[V + 1], bya[V], byb[V], bza[V], bzb[V];
     {
       T bxv[V];
-      xload(A.bx, q.o[1], q.o[2], bxv);
+      xload(A.bx, q.o[1], q.o[2], bxv, A.one);
 #pragma unroll
       for (int v = 0; v < V; ++v) {
         bya[v] = b[0][v] - (f[0][v + 1] - f[0][v]);
@@ -436,7 +442,7 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) lrev_
     x_centre<T, V>(bxe, bya, byb, bza, bzb, B);
   }
 #pragma unroll
-  for (int c = 2; c < 5; ++c) xload(A.u[c], q.o[1], q.o[2], u[c]);
+  for (int c = 2; c < 5; ++c) xload(A.u[c], q.o[1], q.o[2], u[c], A.one);
   T un[V][5];
   fluid_x_core<T, V, NT>(sm, tid, q.tl, q.tr, u, B, gamma, hdt, qdt, un);
   x_store_u_and_cmax<real, T, V>(A, q, un, B);

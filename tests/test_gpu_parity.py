@@ -417,7 +417,7 @@ def test_b_pair_ring_march_fp64(B, bring, bc):
                 assert worst(e) <= TOL64, (bring, bc, seg, d, rev, e)
 
 
-@pytest.mark.parametrize("xpack,xfuse", [(0, 0), (1, 0), (0, 1), (1, 1), (2, 0), (2, 1)])
+@pytest.mark.parametrize("xpack,xfuse", [(0, 0), (1, 0), (0, 1), (1, 1), (2, 0), (2, 1), (3, 1), (3, 3), (2, 2)])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("shape", [(512, 6, 4), (64, 8, 6), (256, 7, 3), (32, 2, 1), (128, 4, 2)])
 def test_x_kernels_pack_and_fused_reverse(B, shape, prec, xpack, xfuse):
