@@ -92,6 +92,18 @@ int mhd_step(mhd_ctx* ctx, int n, double cfl, double* t_advanced);
  * Used for parity tests and for clipping the last step to a target time.  Does not synchronise. */
 int mhd_step_fixed(mhd_ctx* ctx, int n, double dt);
 
+/* The flow loop of PAPER.md:233-243 up to a target time, with the stop test on the device: repeat
+ * { c_max; dt = min(cfl / c_max, (t_end - t) / 2); six L_i; t += 2 dt } until t = t_end (reading R14: the last
+ * step is shortened to land on t_end, and t is then set to t_end exactly) or max_steps steps were taken.
+ * t and t_end are times since mhd_set_state, in grid units.  dt, t and the clipping never leave the GPU
+ * between steps (the paper reads dt back every step); the host enqueues batches of steps sized
+ * from the last dt and reads (t, steps) back once per batch, so the call synchronises a few times.
+ * *steps_done (may be NULL) = steps that advanced time, *t_reached (may be NULL) = t afterwards; the step
+ * index advances by *steps_done.  MHD_EINVAL for cfl <= 0, max_steps < 0 or a NaN t_end; MHD_ENOSTATE before
+ * mhd_set_state; MHD_ENONFINITE if a reduction was poisoned (the state is then whatever the last batch left). */
+int mhd_run_until(mhd_ctx* ctx, double t_end, double cfl, long long max_steps, long long* steps_done,
+                  double* t_reached);
+
 /* One operator of the step, for per-operator parity tests: op = MHD_OP_FLUID (fluid_d, Algorithm 1,
  * PAPER.md:273-285), MHD_OP_BPAIR (B_{t1->d} then B_{t2->d}, or t2 then t1 if reverse != 0;
  * Algorithm 2), MHD_OP_SWEEP_FORWARD / MHD_OP_SWEEP_REVERSE (L_d, PAPER.md:162,
@@ -111,12 +123,22 @@ int mhd_get_time(mhd_ctx* ctx, double* t);
  * NULL.  Synchronises. */
 int mhd_diagnostics(mhd_ctx* ctx, double sums[8], double* max_abs_divb);
 
-/* Tuning knobs, all optional: key "segment" = cells per thread along the sweep for the marching
- * kernels (0 = whole pencil), "block" = threads per block of the generic kernels, "path" = 0 auto |
- * 1 generic kernels only, "btile" = tile shape of the y/z B-pair kernel (0 off, 1 = 32x8 default, 2 = 64x8,
- * 3 = 64x4, 4 = 128x4), "ftma" = stages of the TMA bulk-copy ring of the y/z fluid kernel (0 off, 4, 6
- * default, 8).
- * Unknown keys return MHD_EINVAL. */
+/* Tuning knobs, all optional; none changes what is computed beyond rounding order inside the stated tolerances.
+ *   "graph"   -1 auto (default: grids of <= 2^22 cells) | 0 | 1: replay whole steps of mhd_step / mhd_run_until
+ *             as CUDA graphs (small grids are bound by launch latency)
+ *   "path"    0 auto (default) | 1 generic marching kernels only (any extents, both BCs)
+ *   "segment" cells per block along the sweep for the marching kernels (-1 auto, 0 = whole pencil)
+ *   "block"   threads per block of the generic kernels (multiple of 32 in [32, 256])
+ *   "pack"    fluid y/z ring kernel: 0 off | 1 auto (default; fp32: two pencils per thread in packed f32x2
+ *             arithmetic) | 128 | 256 columns per block
+ *   "bring"   B-pair y/z ring kernel: 0 off | 1 auto (default) | 128 | 256 columns per block
+ *   "ftma"    stages of the older TMA-ring y/z fluid kernel (0 off, 4, 6, 8); used when "pack" = 0
+ *   "btile"   tile shape of the tile-march y/z B-pair kernel (0 off, 1 = 32x8, 2 = 64x8, 3 = 64x4, 4 = 128x4);
+ *             used when "bring" = 0
+ *   "btma", "bstages"  TMA variant of the tile march (0 off) and its ring depth (4, 6, 8)
+ *   "xpack"   x kernels: 0 scalar mhd_x.cuh | 1 all packed | 2 all lane-pack scalar | 3 packed fluid_x only (default)
+ *   "xfuse"   reverse L_x in one kernel: 0 off | 1 fp32 only (default) | 2 always | 3 fp32, packed
+ * Unknown keys and out-of-range values return MHD_EINVAL. */
 int mhd_set_option(mhd_ctx* ctx, const char* key, long long value);
 
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches claim). */

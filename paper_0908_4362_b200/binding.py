@@ -44,6 +44,7 @@ SIGNATURES = {
     "mhd_cfl_dt": (c_int, [c_void_p, c_double, POINTER(c_double), POINTER(c_double)]),
     "mhd_step": (c_int, [c_void_p, c_int, c_double, POINTER(c_double)]),
     "mhd_step_fixed": (c_int, [c_void_p, c_int, c_double]),
+    "mhd_run_until": (c_int, [c_void_p, c_double, c_double, c_longlong, POINTER(c_longlong), POINTER(c_double)]),
     "mhd_apply": (c_int, [c_void_p, c_int, c_int, c_int, c_double]),
     "mhd_get_step_index": (c_int, [c_void_p, POINTER(c_longlong)]),
     "mhd_set_step_index": (c_int, [c_void_p, c_longlong]),
@@ -67,6 +68,7 @@ mhd_get_state = _lib.mhd_get_state
 mhd_cfl_dt = _lib.mhd_cfl_dt
 mhd_step = _lib.mhd_step
 mhd_step_fixed = _lib.mhd_step_fixed
+mhd_run_until = _lib.mhd_run_until
 mhd_apply = _lib.mhd_apply
 mhd_get_step_index = _lib.mhd_get_step_index
 mhd_set_step_index = _lib.mhd_set_step_index
@@ -170,6 +172,12 @@ class Solver:
 
     def step_fixed(self, n, dt):
         self._check(mhd_step_fixed(self._h, int(n), float(dt)))
+
+    def run_until(self, t_end, cfl, max_steps=1 << 40):
+        """-> (steps taken, time reached); the stop test and the last-step clipping run on the device"""
+        n, t = c_longlong(), c_double()
+        self._check(mhd_run_until(self._h, float(t_end), float(cfl), int(max_steps), byref(n), byref(t)))
+        return n.value, t.value
 
     def apply(self, op, d, reverse, dt):
         self._check(mhd_apply(self._h, int(op), int(d), int(bool(reverse)), float(dt)))

@@ -21,6 +21,20 @@
 
 using namespace mhd;
 
+// One whole step (dt kernel + the operator launches of a double sweep) captured as a CUDA graph.  A step leaves
+// every ping-pong pointer where it found it (each field is swapped an even number of times), so a graph captured
+// at step index s can be replayed at every later step with the same index mod 3, the same pointer assignment,
+// the same cfl and the same state of the reduction flags.  For grids of a few thousand to a few million cells
+// a step is bound by launch latency (13 launches of a few microseconds each); replaying it as one graph removes
+// most of that.
+struct StepGraph {
+  cudaGraphExec_t exec;
+  double cfl;
+  void* cur[8];
+  long long launches;       // kernel launches inside the graph
+  bool acc_valid, fin_valid, acc_dirty;   // flags after the step
+};
+
 struct mhd_ctx {
   int n[3];
   double gamma;
@@ -47,11 +61,20 @@ struct mhd_ctx {
   long long launches;
   // options
   int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages, opt_pack, opt_bring, opt_xpack, opt_xfuse;
+  int opt_graph;           // -1 auto (small grids), 0 never, 1 always: replay whole steps as CUDA graphs
+  StepGraph graphs[64];    // one per (step index mod 3, reduction flags, clip)
   int sm_count;
   char err[512];
 };
 
 static thread_local char g_create_err[256] = "";
+
+static void drop_graphs(mhd_ctx* c) {
+  for (StepGraph& g : c->graphs) {
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    g.exec = nullptr;
+  }
+}
 
 static int fail(mhd_ctx* c, int code, const char* fmt, ...) {
   va_list ap;
@@ -116,6 +139,7 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_bring = 1;
   c->opt_xpack = 3;
   c->opt_xfuse = 1;
+  c->opt_graph = -1;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -182,6 +206,7 @@ extern "C" int mhd_bind(mhd_ctx* c, void* device_workspace, size_t bytes, void* 
 extern "C" int mhd_destroy(mhd_ctx* c) {
   if (!c) return MHD_OK;
   if (c->stream_set) cudaStreamSynchronize(c->stream);
+  drop_graphs(c);
   if (c->owns_ws && c->ws) cudaFree(c->ws);
   if (c->owns_stream && c->stream_set) cudaStreamDestroy(c->stream);
   delete c;
@@ -241,7 +266,7 @@ static SweepGeom<real> make_geom(const mhd_ctx* c, int d) {
     const long long pencils = (long long)g.na * g.nb;
     const long long want = (long long)c->sm_count * 2048;      // resident-thread capacity
     seg = g.nd;
-    while (seg > 32 && pencils * ((g.nd + seg - 1) / seg) < want) seg = (seg + 1) / 2;
+    while (seg > 8 && pencils * ((g.nd + seg - 1) / seg) < want) seg = (seg + 1) / 2;
   }
   if (seg == 0 || seg > g.nd) seg = g.nd;
   g.seg = seg;
@@ -262,7 +287,7 @@ static bool yz_ok(const mhd_ctx* c, int d) {
 static int pick_segment(int nd, long long pencil_blocks, long long slots, int halo) {
   int best_seg = nd;
   double best = 1e300;
-  for (int nseg = 1; nseg <= 16 && nd / nseg >= 32; ++nseg) {
+  for (int nseg = 1; nseg <= 64 && nd / nseg >= 8; ++nseg) {
     const int seg = ((nd + nseg - 1) / nseg + 3) & ~3;              // multiple of 4 (the marches are unrolled by 4)
     const long long blocks = pencil_blocks * ((nd + seg - 1) / seg);
     const double cost = (double)((blocks + slots - 1) / slots) * (seg + halo);
@@ -677,7 +702,7 @@ static int read_scalars(mhd_ctx* c, Scalars* h) {
 }
 
 // make sc->cmax / sc->dt current: run the reduction only if no fused one is pending
-static int refresh_dt(mhd_ctx* c, double cfl, int advance) {
+static int refresh_dt(mhd_ctx* c, double cfl, int advance, int clip = 0) {
   int reuse = 0;
   if (c->fin_valid) reuse = 1;
   else if (!c->acc_valid) {
@@ -686,12 +711,62 @@ static int refresh_dt(mhd_ctx* c, double cfl, int advance) {
     if ((rc = BY_PRECISION(c, launch_cfl<float>(c), launch_cfl<double>(c)))) return rc;
     c->acc_dirty = true;
   }
-  dt_from_cmax_kernel<<<1, 1, 0, c->stream>>>(c->sc, cfl, advance, reuse);
+  dt_from_cmax_kernel<<<1, 1, 0, c->stream>>>(c->sc, cfl, advance, reuse, clip);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
   if (!reuse) c->acc_dirty = false;            // finalising re-arms the accumulator
   c->acc_valid = false;
   c->fin_valid = true;
+  return MHD_OK;
+}
+
+static bool graphs_wanted(const mhd_ctx* c) {
+  if (c->opt_graph >= 0) return c->opt_graph != 0;
+  return c->N <= ((size_t)1 << 22);
+}
+
+// one step: c_max -> dt (kept on the device) -> six L_i, directly or as a replayed CUDA graph
+static int step_once(mhd_ctx* c, double cfl, int clip) {
+  int rc;
+  if (!graphs_wanted(c)) {
+    if ((rc = refresh_dt(c, cfl, 1, clip))) return rc;
+    return double_sweep(c);
+  }
+  const int key = (int)(((c->step_index % 3) + 3) % 3) | (c->acc_valid ? 4 : 0) | (c->fin_valid ? 8 : 0) |
+                  (c->acc_dirty ? 16 : 0) | (clip ? 32 : 0);
+  StepGraph& g = c->graphs[key];
+  bool hit = g.exec != nullptr && g.cfl == cfl;
+  for (int f = 0; hit && f < 8; ++f) hit = g.cur[f] == c->cur[f];
+  if (!hit) {
+    if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+    const long long step0 = c->step_index, launches0 = c->launches;
+    void* cur0[8];
+    memcpy(cur0, c->cur, sizeof(cur0));
+    CUDA_TRY(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    rc = refresh_dt(c, cfl, 1, clip);
+    if (!rc) rc = double_sweep(c);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(c, MHD_ECUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
+    const cudaError_t e2 = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e2 != cudaSuccess) { g.exec = nullptr; return fail(c, MHD_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e2)); }
+    for (int f = 0; f < 8; ++f)
+      if (c->cur[f] != cur0[f]) {          // cannot happen (even number of swaps per field); never replay such a graph
+        cudaGraphExecDestroy(g.exec); g.exec = nullptr;
+        return fail(c, MHD_ECUDA, "internal: a step did not restore the ping-pong pointers");
+      }
+    g.cfl = cfl;
+    memcpy(g.cur, cur0, sizeof(cur0));
+    g.launches = c->launches - launches0;
+    g.acc_valid = c->acc_valid; g.fin_valid = c->fin_valid; g.acc_dirty = c->acc_dirty;
+    c->step_index = step0; c->launches = launches0;   // the capture recorded the work; the launch below does it
+  }
+  CUDA_TRY(c, cudaGraphLaunch(g.exec, c->stream));
+  c->acc_valid = g.acc_valid; c->fin_valid = g.fin_valid; c->acc_dirty = g.acc_dirty;
+  c->launches += g.launches;
+  c->step_index++;
   return MHD_OK;
 }
 
@@ -715,10 +790,8 @@ extern "C" int mhd_step(mhd_ctx* c, int n, double cfl, double* t_advanced) {
   int rc;
   reset_call_kernel<<<1, 1, 0, c->stream>>>(c->sc);
   c->launches++;
-  for (int it = 0; it < n; ++it) {
-    if ((rc = refresh_dt(c, cfl, 1))) return rc;
-    if ((rc = double_sweep(c))) return rc;
-  }
+  for (int it = 0; it < n; ++it)
+    if ((rc = step_once(c, cfl, 0))) return rc;
   CUDA_TRY(c, cudaGetLastError());
   if (t_advanced) {
     Scalars h;
@@ -726,6 +799,45 @@ extern "C" int mhd_step(mhd_ctx* c, int n, double cfl, double* t_advanced) {
     *t_advanced = h.t_call;
     return check_poison(c, h);
   }
+  return MHD_OK;
+}
+
+// The flow loop of PAPER.md:233-243 with the stop test on the device.  The paper reads
+// dt back to the host every step; here dt, t and the clipping of the last step stay in the
+// scalar block, the host enqueues batches of steps sized from the last dt so that a batch cannot pass t_end
+// unless dt grows by more than 10 % inside it (steps enqueued past t_end run with dt = 0 and change nothing),
+// and reads (t, steps) back once per batch.
+extern "C" int mhd_run_until(mhd_ctx* c, double t_end, double cfl, long long max_steps, long long* steps_done,
+                             double* t_reached) {
+  if (!c) return MHD_EINVAL;
+  if (!(cfl > 0.0) || max_steps < 0 || !(t_end == t_end)) return fail(c, MHD_EINVAL, "mhd_run_until: bad argument");
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "mhd_run_until: no state set");
+  int rc;
+  Scalars h;
+  begin_run_kernel<<<1, 1, 0, c->stream>>>(c->sc, t_end);
+  c->launches++;
+  if ((rc = refresh_dt(c, cfl, 0))) return rc;          // first dt estimate (the first step reuses this c_max)
+  if ((rc = read_scalars(c, &h))) return rc;
+  if ((rc = check_poison(c, h))) return rc;
+  const long long step0 = c->step_index;
+  long long done = 0;
+  double dt_est = h.dt;
+  while (h.t_total < t_end && done < max_steps) {
+    const double est = (t_end - h.t_total) / (2.0 * dt_est);
+    long long batch = est < 4.0e9 ? (long long)(0.9 * est) : 4000000000ll;
+    if (batch < 1) batch = 1;
+    if (batch > 512) batch = 512;
+    if (batch > max_steps - done) batch = max_steps - done;
+    for (long long it = 0; it < batch; ++it)
+      if ((rc = step_once(c, cfl, 1))) return rc;
+    if ((rc = read_scalars(c, &h))) return rc;
+    c->step_index = step0 + h.steps_real;               // steps enqueued past t_end did nothing: do not count them
+    if ((rc = check_poison(c, h))) return rc;
+    done = h.steps_real;
+    dt_est = h.dt_last > 0.0 ? h.dt_last : dt_est;
+  }
+  if (steps_done) *steps_done = done;
+  if (t_reached) *t_reached = h.t_total;
   return MHD_OK;
 }
 
@@ -812,6 +924,7 @@ extern "C" int mhd_diagnostics(mhd_ctx* c, double sums[8], double* max_abs_divb)
 
 extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   if (!c || !key) return MHD_EINVAL;
+  drop_graphs(c);                                       // captured steps bake in the kernel choice
   if (!strcmp(key, "segment")) { if (value < -1) return fail(c, MHD_EINVAL, "segment < -1"); c->opt_segment = (int)value; return MHD_OK; }
   if (!strcmp(key, "block")) {
     if (value < 32 || value > 256 || (value & 31)) return fail(c, MHD_EINVAL, "block must be a multiple of 32 in [32,256]");
@@ -825,6 +938,7 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   if (!strcmp(key, "pack")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "pack must be 0, 1, 128 or 256"); c->opt_pack = (int)value; return MHD_OK; }
   if (!strcmp(key, "xpack")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 0..3"); c->opt_xpack = (int)value; return MHD_OK; }
   if (!strcmp(key, "xfuse")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xfuse must be 0, 1 (fp32 only), 2 (always) or 3 (fp32, packed)"); c->opt_xfuse = (int)value; return MHD_OK; }
+  if (!strcmp(key, "graph")) { if (value < -1 || value > 1) return fail(c, MHD_EINVAL, "graph must be -1 (auto), 0 or 1"); c->opt_graph = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
   return fail(c, MHD_EINVAL, "unknown option '%s'", key);
 }

@@ -192,11 +192,17 @@ struct Scalars {
   unsigned long long cmax_bits;    // reduction target
   int nonfinite;                   // sticky flag: a reduction saw NaN/Inf or c_max <= 0
   int pad;
+  double t_end;                    // target time of mhd_run_until (time since set_state); unused unless clip = 1
+  double dt_last;                  // last positive dt (the host sizes the next batch of mhd_run_until from it)
+  long long steps_real;            // steps of the current mhd_run_until call that advanced time (dt > 0)
 };
 
 // one thread: dt = cfl / c_max, t += 2 dt; re-arms the reduction
 // reuse = 0: finalize the reduction (cmax <- accumulator, accumulator re-armed); 1: s->cmax is already final
-__global__ void dt_from_cmax_kernel(Scalars* s, double cfl, int advance, int reuse) {
+// clip = 1 (mhd_run_until): dt = min(cfl / c_max, (t_end - t) / 2) (reading R14: the loop of PAPER.md:233-243 stops
+// at a given time, the last step is shortened to land on it); a clipped step sets t = t_end exactly, and once
+// t >= t_end every further step gets dt = 0, which makes all six operators exact no-ops (u - 0 * flux = u).
+__global__ void dt_from_cmax_kernel(Scalars* s, double cfl, int advance, int reuse, int clip) {
   double cm = s->cmax;
   if (!reuse) {
     cm = __longlong_as_double((long long)s->cmax_bits);
@@ -206,9 +212,24 @@ __global__ void dt_from_cmax_kernel(Scalars* s, double cfl, int advance, int reu
   double dt = 0.0;
   if (!(cm > 0.0) || isinf(cm) || isnan(cm)) s->nonfinite = 1;
   else dt = cfl / cm;
+  if (clip && advance) {
+    const double rem = 0.5 * (s->t_end - s->t_total);
+    if (!(rem > 0.0)) dt = 0.0;
+    else if (dt >= rem) {
+      s->dt = rem;
+      s->dt_last = rem;
+      s->t_call += s->t_end - s->t_total;
+      s->t_total = s->t_end;
+      s->steps_real += 1;
+      return;
+    }
+    if (dt > 0.0) { s->steps_real += 1; s->dt_last = dt; }
+  }
   s->dt = dt;
   if (advance) { s->t_total += 2.0 * dt; s->t_call += 2.0 * dt; }
 }
+
+__global__ void begin_run_kernel(Scalars* s, double t_end) { s->t_call = 0.0; s->t_end = t_end; s->steps_real = 0; }
 
 __global__ void set_dt_kernel(Scalars* s, double dt, int nsteps) {
   s->dt = dt;
