@@ -42,4 +42,20 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                : "memory");
 }
 
+// One lane of a fully converged warp.  ptxas recognises the elect.sync predicate: a cp.async.bulk guarded by it
+// becomes one UBLKCP with operands in uniform registers.  Guarded by a lane-index test instead, every copy is
+// wrapped in an ELECT / 5 x R2UR.BROADCAST / BRA.U.ANY loop over the active lanes (10 instructions per copy,
+// measured: 12 % of the B-pair ring kernel's issued instructions, profiles/r01_c4_step_ncu_full_c.md).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "elect.sync _|p, 0xffffffff;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 }  // namespace mhd

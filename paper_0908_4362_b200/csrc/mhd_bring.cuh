@@ -70,7 +70,8 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   uint64_t* full = reinterpret_cast<uint64_t*>(ring + D * RG::STAGE);
   uint64_t* empty = full + D;
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // the same value, warp-uniform for the compiler too
   const int x0 = blockIdx.x * TXB, o = blockIdx.y;
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
@@ -82,40 +83,37 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   }
   __syncthreads();
 
-  // ---- producer duty: lane c < NCOPY of the warp on duty issues copy c of a stage ---------------------
-  const real* src = nullptr;
-  int dst = 0, late = 0;
-  uint32_t nbytes = TXB * sizeof(real);
-  {
-    const int om = map_index1(o - 1, A.no, A.bc), op = map_index1(o + 1, A.no, A.bc);
-    int xoff = x0;
-    switch (lane) {
-      case 0: src = A.u[0] + (size_t)om * A.so; dst = 0 * P + CH; break;
-      case 1: src = A.u[0] + (size_t)o * A.so;  dst = 1 * P + CH; break;
-      case 2: src = A.u[0] + (size_t)op * A.so; dst = 2 * P + CH; break;
-      case 3: src = A.u[1] + (size_t)om * A.so; dst = 3 * P + CH; break;
-      case 4: src = A.u[1] + (size_t)o * A.so;  dst = 4 * P + CH; break;
-      case 5: src = A.u[1] + (size_t)op * A.so; dst = 5 * P + CH; break;
-      case 6: src = A.bx + (size_t)o * A.so;    dst = 6 * P + CH; break;
-      case 7: src = A.bo + (size_t)o * A.so;    dst = 7 * P + CH; break;
-      case 8: src = A.bo + (size_t)op * A.so;   dst = 8 * P + CH; break;
-      case 9: src = A.bd + (size_t)o * A.so;    dst = 9 * P + CH; late = 4; break;
-      case 10: src = A.u[0] + (size_t)o * A.so; dst = 1 * P;            xoff = (xl / CH) * CH; nbytes = 16; break;
-      case 11: src = A.u[0] + (size_t)o * A.so; dst = 1 * P + CH + TXB; xoff = (xr / CH) * CH; nbytes = 16; break;
-      case 12: src = A.u[1] + (size_t)o * A.so; dst = 4 * P;            xoff = (xl / CH) * CH; nbytes = 16; break;
-      case 13: src = A.u[1] + (size_t)o * A.so; dst = 4 * P + CH + TXB; xoff = (xr / CH) * CH; nbytes = 16; break;
-      default: src = A.bx + (size_t)o * A.so;   dst = 6 * P + CH + TXB; xoff = (xr / CH) * CH; nbytes = 16; break;
-    }
-    src += xoff;
-  }
-  auto produce = [&](int itp) {                           // called by one whole warp
+  // ---- producer duty: one elected lane of the warp on duty issues the NCOPY copies of a stage; every operand is
+  // warp-uniform (block indices, kernel parameters, the march step), so they are straight-line UBLKCPs (mhd_async.cuh)
+  const int om_off = map_index1(o - 1, A.no, A.bc) * A.so, o_off = o * A.so, op_off = map_index1(o + 1, A.no, A.bc) * A.so;
+  const int cl = (xl / CH) * CH + o_off, cr = (xr / CH) * CH + o_off;     // the 16-byte chunks holding columns x0-1, x0+TXB of row o
+  auto produce = [&](int itp) {                           // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
-    if (lane < RG::NCOPY) {
-      const int od = map_index1(n0 - 4 + itp - late, A.nd, A.bc) * A.sd;
-      if (lane == 0) mbar_expect_tx(&full[s], RG::BYTES);
-      __syncwarp((1u << RG::NCOPY) - 1u);
-      bulk_g2s(ring + s * RG::STAGE + dst, src + od, nbytes, &full[s]);
+    if (elect_one()) {
+      const int od = map_index1(n0 - 4 + itp, A.nd, A.bc) * A.sd;
+      const int odl = map_index1(n0 - 8 + itp, A.nd, A.bc) * A.sd;        // B_d of the cell finished at this step
+      real* st = ring + s * RG::STAGE;
+      uint64_t* bar = &full[s];
+      constexpr uint32_t RB = TXB * sizeof(real);
+      const real* rho = A.u[0] + od;
+      const real* md = A.u[1] + od;
+      mbar_expect_tx(bar, RG::BYTES);
+      bulk_g2s(st + 0 * P + CH, rho + om_off + x0, RB, bar);
+      bulk_g2s(st + 1 * P + CH, rho + o_off + x0, RB, bar);
+      bulk_g2s(st + 2 * P + CH, rho + op_off + x0, RB, bar);
+      bulk_g2s(st + 3 * P + CH, md + om_off + x0, RB, bar);
+      bulk_g2s(st + 4 * P + CH, md + o_off + x0, RB, bar);
+      bulk_g2s(st + 5 * P + CH, md + op_off + x0, RB, bar);
+      bulk_g2s(st + 6 * P + CH, A.bx + od + o_off + x0, RB, bar);
+      bulk_g2s(st + 7 * P + CH, A.bo + od + o_off + x0, RB, bar);
+      bulk_g2s(st + 8 * P + CH, A.bo + od + op_off + x0, RB, bar);
+      bulk_g2s(st + 9 * P + CH, A.bd + odl + o_off + x0, RB, bar);
+      bulk_g2s(st + 1 * P, rho + cl, 16, bar);
+      bulk_g2s(st + 1 * P + CH + TXB, rho + cr, 16, bar);
+      bulk_g2s(st + 4 * P, md + cl, 16, bar);
+      bulk_g2s(st + 4 * P + CH + TXB, md + cr, 16, bar);
+      bulk_g2s(st + 6 * P + CH + TXB, A.bx + od + cr, 16, bar);
     }
     __syncwarp();
   };

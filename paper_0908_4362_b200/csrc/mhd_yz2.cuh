@@ -52,7 +52,8 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   uint64_t* full = reinterpret_cast<uint64_t*>(ring + D * RG::STAGE);
   uint64_t* empty = full + D;
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // the same value, warp-uniform for the compiler too
   const int x0 = blockIdx.x * TXB;
   const int o = blockIdx.y;
   const int n0 = blockIdx.z * A.seg;
@@ -64,29 +65,28 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   }
   __syncthreads();
 
-  // ---- producer duty: lane c < 10 of the warp on duty issues copy c of a stage -----------------------
-  const real* src = nullptr;                             // source row of my copy at march position 0
-  int dst = 0, qshift = 0;
-  uint32_t nbytes = TXB * sizeof(real);
-  {
-    const int rowbase = x0 + o * A.so;
-    const int op_off = (map_index1(o + 1, A.no, A.bc) - o) * A.so;
-    const int xn = map_index1(x0 + TXB, A.nx, A.bc);     // B_x at x0+TXB lives in this 16-byte chunk
-    if (lane < 5) { src = A.u[lane] + rowbase; dst = lane * RG::ROW; }
-    else if (lane == 5) { src = A.bd + rowbase; dst = 5 * RG::ROW; qshift = 1; }
-    else if (lane == 6) { src = A.bo + rowbase; dst = 6 * RG::ROW; }
-    else if (lane == 7) { src = A.bo + rowbase + op_off; dst = 7 * RG::ROW; }
-    else if (lane == 8) { src = A.bx + rowbase; dst = 8 * RG::ROW; }
-    else if (lane == 9) { src = A.bx + (xn / RG::CH) * RG::CH + o * A.so; dst = 9 * RG::ROW; nbytes = 16; }
-  }
-  auto produce = [&](int itp) {                          // called by one whole warp
+  // ---- producer duty: one elected lane of the warp on duty issues the 10 copies of a stage; every operand is
+  // warp-uniform (block indices, kernel parameters, the march step), so the copies are straight-line UBLKCPs ------
+  const int rowbase = x0 + o * A.so;
+  const int op_off = (map_index1(o + 1, A.no, A.bc) - o) * A.so;
+  const int xchunk = (map_index1(x0 + TXB, A.nx, A.bc) / RG::CH) * RG::CH + o * A.so;   // B_x at x0+TXB lives in this 16-byte chunk
+  auto produce = [&](int itp) {                          // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
-    if (lane < 10) {
-      const int od = map_index1(n0 - 3 + itp + qshift, A.nd, A.bc) * A.sd;
-      if (lane == 0) mbar_expect_tx(&full[s], RG::BYTES);
-      __syncwarp(0x3ffu);
-      bulk_g2s(ring + s * RG::STAGE + dst, src + od, nbytes, &full[s]);
+    if (elect_one()) {
+      const int q = n0 - 3 + itp;
+      const int od = map_index1(q, A.nd, A.bc) * A.sd;
+      const int od1 = map_index1(q + 1, A.nd, A.bc) * A.sd;
+      real* st = ring + s * RG::STAGE;
+      constexpr uint32_t RB = TXB * sizeof(real);
+      mbar_expect_tx(&full[s], RG::BYTES);
+#pragma unroll
+      for (int k = 0; k < 5; ++k) bulk_g2s(st + k * RG::ROW, A.u[k] + od + rowbase, RB, &full[s]);
+      bulk_g2s(st + 5 * RG::ROW, A.bd + od1 + rowbase, RB, &full[s]);
+      bulk_g2s(st + 6 * RG::ROW, A.bo + od + rowbase, RB, &full[s]);
+      bulk_g2s(st + 7 * RG::ROW, A.bo + od + rowbase + op_off, RB, &full[s]);
+      bulk_g2s(st + 8 * RG::ROW, A.bx + od + rowbase, RB, &full[s]);
+      bulk_g2s(st + 9 * RG::ROW, A.bx + od + xchunk, 16, &full[s]);
     }
     __syncwarp();
   };
