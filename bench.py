@@ -31,12 +31,23 @@ WORKLOADS = {
     "c5": ("turbulence", 512, "f64", "configs[4]: same seeded state, 512^3, fp64, periodic, cfl 0.8"),
     "c3": ("blast3d", 256, "f32", "configs[2]: 3-D MHD blast wave, 256^3, fp32, periodic, cfl 0.8"),
     "small": ("turbulence", 128, "f32", "reduced 128^3 fp32 turbulence-like state (not a BASELINE config)"),
+    # the paper's own 3-D blast wave (E6, B = (1,1,1)/sqrt 3) at its largest size; Table 3 has its ms/step
+    "e6": ("blast3d_paper", 128, "f32", "paper E6: 3-D blast wave, 128^3, fp32, B=(1,1,1)/sqrt(3) (PAPER.md:539-559; not a BASELINE config)"),
 }
+# BASELINE.md section 1, the paper's own number for the same workload on another machine (context, not the target):
+# 128^3 fp32 3-D blast on a GTX 480, 161.33 ms/step (Table 3) = 13.0 M cell-updates/s
+PAPER_RATE = {"e6": 128 ** 3 / 161.33e-3}
+
+
+def _gen(inputs, gen, n, **kw):
+    if gen == "turbulence":
+        return inputs.turbulence(n, **kw)
+    return inputs.blast3d(n, paper_field=(gen == "blast3d_paper"), **kw)
 ALGO_WORDS_STEP = 96          # ideal: each of the six L_i reads 8 fields and writes 8
 CFL = 0.8
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/r01_c4_step_ncu_full_c.md, profiles/r01_c5_step_ncu_full_b.md); None where no capture exists
-NCU_TRAFFIC = {("c4", "fluid_yz"): 7.059e9, ("c5", "fluid_yz"): 14.07e9}
+NCU_TRAFFIC = {("c4", "fluid_yz"): 7.058e9, ("c5", "fluid_yz"): 14.10e9}
 
 
 def peaks():
@@ -94,7 +105,7 @@ def make_state(gen, n, prec, device):
     import torch
     from paper_0908_4362_b200 import inputs
     kw = dict(xp=torch, xp_kw={"device": device})
-    f, meta = (inputs.turbulence(n, **kw) if gen == "turbulence" else inputs.blast3d(n, **kw))
+    f, meta = _gen(inputs, gen, n, **kw)
     dt = torch.float32 if prec == "f32" else torch.float64
     out = [a.to(dt).contiguous() for a in f]
     del f
@@ -106,7 +117,7 @@ def oracle_rate(gen, prec, budget_s=12.0, n=96):
     """the oracle as it stands, timed on the host cores on a bounded sample of the workload"""
     import oracle
     from paper_0908_4362_b200 import inputs
-    f, meta = (inputs.turbulence(n) if gen == "turbulence" else inputs.blast3d(n))
+    f, meta = _gen(inputs, gen, n)
     dt = np.float32 if prec == "f32" else np.float64
     st = [np.array(a, dtype=dt) for a in f]
     oracle.run(st, meta["gamma"], meta["bc"], 0, 1, CFL)            # page in / warm caches
@@ -128,7 +139,7 @@ def run_reference(args, rank, world):
     import oracle
     from paper_0908_4362_b200 import inputs
     ns = 96 if n >= 96 else n
-    f, meta = (inputs.turbulence(ns) if gen == "turbulence" else inputs.blast3d(ns))
+    f, meta = _gen(inputs, gen, ns)
     dt = np.float32 if prec == "f32" else np.float64
     st = [np.array(a, dtype=dt) for a in f]
     k0 = 0
@@ -300,7 +311,8 @@ def main():
         out = {
             "metric": "MHD cell-updates/sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
+            "scaling": "weak", "vs_baseline": (value / PAPER_RATE[args.workload] if args.workload in PAPER_RATE else None),
+            "dtype": prec, "data": "synthetic",
             "config": {"workload": f"{args.workload}: {desc}", "grid": [n, n, n], "cfl": CFL, "gamma": meta["gamma"],
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"state {8 * N * esize / 1e9:.2f} GB per copy >> 126 MB L2 (inputs larger than L2, no flush needed)",

@@ -126,7 +126,9 @@ def orszag_tang(n=256, nz=1):
 # ----------------------------------------------------------------------------------------------
 # config 3: 3-D blast wave (BASELINE.json configs[2]; PAPER.md:539-559 for rho, p, r, gamma)
 # ----------------------------------------------------------------------------------------------
-def blast3d(n=256, xp=np, xp_kw=None):
+def blast3d(n=256, xp=np, xp_kw=None, paper_field=False):
+    """paper_field=True: the paper's own experiment E6, B = (1,1,1)/sqrt(3) instead of
+    BASELINE.json's (1,1,0)/sqrt(2); same rho, p, radius"""
     xp_kw = xp_kw or {}
     gamma = 5.0 / 3.0
     c = (xp.arange(n, dtype=xp.float64, **xp_kw) + 0.5) / n - 0.5
@@ -136,11 +138,34 @@ def blast3d(n=256, xp=np, xp_kw=None):
     p = xp.where(r2 < 0.1 * 0.1, 10.0 * one, 0.1 * one)
     rho = one
     z = xp.zeros(shape, dtype=xp.float64, **xp_kw)
+    if paper_field:
+        b = 1.0 / math.sqrt(3.0)
+        bx, by, bz = b * one, b * one, b * one
+    else:
+        b = 1.0 / math.sqrt(2.0)
+        bx, by, bz = b * one, b * one, z * 1.0
+    E = p / (gamma - 1.0) + 0.5 * (bx * bx + by * by + bz * bz)       # v = 0, uniform B
+    return [rho, z, z * 1.0, z * 1.0, E, bx, by, bz], dict(
+        gamma=gamma, bc=PERIODIC, name="blast3d_paper" if paper_field else "blast3d", box=(1.0, 1.0, 1.0))
+
+
+# ----------------------------------------------------------------------------------------------
+# the paper's experiment E4: 2-D blast wave: rho = 1, p = 10 inside r < 0.1 of the centre of the
+# unit square, 0.1 outside, B = (1/sqrt 2, 1/sqrt 2, 0), gamma = 5/3, v = 0; periodic.  Initial data only
+# (SURVEY.md 8(f) rank 3); the stray "p = 5/(12 pi)" of eq (48) is a garble from the Orszag-Tang block (R19).
+# ----------------------------------------------------------------------------------------------
+def blast2d(n=512, nz=1):
+    gamma = 5.0 / 3.0
+    c = (np.arange(n, dtype=np.float64) + 0.5) / n - 0.5
+    r2 = c[None, None, :] ** 2 + c[None, :, None] ** 2 + np.zeros((nz, 1, 1))
+    one = np.ones((nz, n, n))
+    p = np.where(r2 < 0.1 * 0.1, 10.0 * one, 0.1 * one)
+    z = np.zeros((nz, n, n))
     b = 1.0 / math.sqrt(2.0)
-    bx, by, bz = b * one, b * one, z
-    E = p / (gamma - 1.0) + 0.5 * (bx * bx + by * by)       # v = 0, uniform B
-    return [rho, z, z * 1.0, z * 1.0, E, bx, by, z * 1.0], dict(
-        gamma=gamma, bc=PERIODIC, name="blast3d", box=(1.0, 1.0, 1.0))
+    bx, by = b * one, b * one
+    E = p / (gamma - 1.0) + 0.5 * (bx * bx + by * by)
+    return [one.copy(), z, z.copy(), z.copy(), E, bx, by, z.copy()], dict(
+        gamma=gamma, bc=PERIODIC, name="blast2d", box=(1.0, 1.0, 1.0 / n))
 
 
 # ----------------------------------------------------------------------------------------------
@@ -249,4 +274,4 @@ CONFIGS = {
 
 
 def make(gen: str, **kw):
-    return {"brio_wu": brio_wu, "orszag_tang": orszag_tang, "blast3d": blast3d, "turbulence": turbulence}[gen](**kw)
+    return {"brio_wu": brio_wu, "orszag_tang": orszag_tang, "blast3d": blast3d, "blast2d": blast2d, "turbulence": turbulence}[gen](**kw)

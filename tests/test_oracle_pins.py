@@ -436,3 +436,22 @@ def test_cmax_surfaces_nan():
     f = c64(f)
     f[0][3, 3, 3] = np.nan
     assert math.isnan(oracle.cmax(f, meta["gamma"], meta["bc"]))
+
+
+def test_second_workload_set_generators():
+    """initial data of the paper's E4 / E6: uniform B (div B = 0
+    exactly), v = 0, p jump 10 / 0.1 at r = 0.1, and the oracle keeps the 2-D run 2-D"""
+    from paper_0908_4362_b200 import inputs
+    f, meta = inputs.blast2d(64)
+    g = meta["gamma"]
+    p = (g - 1.0) * (f[4] - 0.5 * (f[5] ** 2 + f[6] ** 2 + f[7] ** 2))
+    assert abs(p.max() - 10.0) < 1e-12 and abs(p.min() - 0.1) < 1e-12
+    assert abs((p > 1).mean() - np.pi * 0.01) < 2e-3            # disc of radius 0.1 in the unit square
+    assert np.all(f[5] == f[5].flat[0]) and np.all(f[6] == f[5].flat[0]) and not f[7].any()
+    st = [a.copy() for a in f]
+    oracle.step_fixed(st, g, meta["bc"], 0, 0.05)
+    assert not st[3].any() and not st[7].any() and np.abs(st[0] - 1).max() > 1e-3
+    f3, m3 = inputs.blast3d(24, paper_field=True)
+    assert np.allclose(f3[5] ** 2 + f3[6] ** 2 + f3[7] ** 2, 1.0)
+    p3 = (m3["gamma"] - 1.0) * (f3[4] - 0.5)
+    assert abs(p3.max() - 10.0) < 1e-12 and abs(p3.min() - 0.1) < 1e-12
