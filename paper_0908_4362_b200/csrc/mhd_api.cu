@@ -350,11 +350,13 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
       if (P == 256) {
         if constexpr (f32) {
           smem = FluidRing<real, 256>::smem_bytes(DR);
-          k = A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 256, DR, true> : fluid_yz_ring_kernel<real, T, 256, DR, false>;
+          k = want_cmax ? (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, true> : fluid_yz_ring_kernel<real, T, 256, DR, false, true>)
+                        : (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, false> : fluid_yz_ring_kernel<real, T, 256, DR, false, false>);
         }
       } else {
         smem = FluidRing<real, 128>::smem_bytes(DR);
-        k = A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 128, DR, true> : fluid_yz_ring_kernel<real, T, 128, DR, false>;
+        k = want_cmax ? (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, true> : fluid_yz_ring_kernel<real, T, 128, DR, false, true>)
+                      : (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, false> : fluid_yz_ring_kernel<real, T, 128, DR, false, false>);
       }
       CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       k<<<grid, P / PackOf<T>::L, smem, c->stream>>>(A);

@@ -38,7 +38,9 @@ namespace mhd {
 
 // real: element type in memory.  T: arithmetic pack (f2 for float, double for double).
 // D ring stages, PF = D - 4 - SLACK steps of prefetch.
-template <class real, class T, int TXB, int D, bool XT1>
+// CM: also reduce c of eq (18) over the updated cells (the last operator of a step); a compile-time switch keeps the
+// reduction out of the instruction stream and the register allocation of the other five launches of a step
+template <class real, class T, int TXB, int D, bool XT1, bool CM>
 __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_ring_kernel(const YZArgs<real> A) {
   using RG = FluidRing<real, TXB>;
   typedef typename PackOf<T>::scalar S;
@@ -147,13 +149,13 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
       const int off = m * A.sd + base;
 #pragma unroll
       for (int k = 0; k < 5; ++k) st_pack(A.uo[k] + off, out[k]);
-      if (A.cmax_bits) {          // last operator of a step: c of eq (18) from the updated cells (B unchanged)
+      if (CM) {                   // last operator of a step: c of eq (18) from the updated cells (B unchanged)
         const unsigned long long b = pack_speed_bits(out, pipe.hb2_out(), A.gamma);
         cbest = b > cbest ? b : cbest;
       }
     }
   }
-  if (A.cmax_bits) {
+  if (CM) {
     cbest = warp_max_u64(cbest);
     if (lane == 0) publish_max(A.cmax_bits, cbest);
   }
