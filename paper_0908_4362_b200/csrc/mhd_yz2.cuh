@@ -21,11 +21,12 @@
 
 namespace mhd {
 
-// Resident blocks per SM the register budget is cut for.  Measured at 512^3 fp32 with the earlier
-// producer-warp version (ms per launch): 168 registers 1.28; 214 registers, no spills, 4 consumer
-// warps per SM 1.96; 128 registers with spills 1.94; 96 registers 3.3.  The scalar kernel: 1.60.
+// Resident blocks per SM the register budget is cut for.  Measured at 512^3 fp32 (ms per launch), current kernel
+// (elected-lane producer, c_max as a template switch): 2 blocks / 184 registers 1.17, 3 blocks / 168 registers, no
+// spills, 1.11 (8 stages x 9.2 KB x 3 blocks = 222 KB of shared memory: the most that fits); 7 stages 1.13.
+// Earlier producer-warp version: 168 registers 1.28; 128 registers with spills 1.94; 96 registers 3.3.
 #ifndef MHD_YZ2_MINB
-#define MHD_YZ2_MINB 2
+#define MHD_YZ2_MINB 3
 #endif
 #ifndef MHD_YZ2_STAGES
 #define MHD_YZ2_STAGES 8
