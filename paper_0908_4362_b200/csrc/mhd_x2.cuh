@@ -327,6 +327,15 @@ __device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const X
 #define MHD_X2_MINB64 2    // fp64: 256-thread blocks
 #endif
 #define MHD_X2_MINB(real, T) (sizeof(real) == 8 ? MHD_X2_MINB64 : (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1))
+// the scalar fp32 B pair and fused reverse L_x have their own budgets
+#ifndef MHD_X2_MINB1_B
+#define MHD_X2_MINB1_B 5
+#endif
+#ifndef MHD_X2_MINB1_L
+#define MHD_X2_MINB1_L 6     // 80 registers: 2.09 ms at 512^3 (5: 96 registers 2.17; 7: 72 registers, spills, 2.15; 8: 2.43)
+#endif
+#define MHD_X2_MINB_B(real, T) (sizeof(real) == 8 ? MHD_X2_MINB64 : (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1_B))
+#define MHD_X2_MINB_L(real, T) (sizeof(real) == 8 ? MHD_X2_MINB64 : (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1_L))
 
 // ---- fluid_x --------------------------------------------------------------------------------------
 template <class real, class T>
@@ -359,7 +368,7 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) fluid
 
 // ---- B_{y->x}, B_{z->x} ------------------------------------------------------------------------------
 template <class real, class T>
-__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) bpair_x2_kernel(const XArgs<real> A) {
+__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB_B(real, T)) bpair_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
   constexpr int NT = X2Block<real>::NT;
@@ -395,7 +404,7 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) bpair
 // Shared memory: 35 slots x NT packs (the B pair uses slots 0..23, the B_x' exchange slot 34,
 // fluid_x slots 0..34; slot 34 is rewritten by fluid_x only two barriers after it was read).
 template <class real, class T>
-__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) lrev_x2_kernel(const XArgs<real> A) {
+__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB_L(real, T)) lrev_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
   constexpr int NT = X2Block<real>::NT;
