@@ -136,7 +136,7 @@ int mhd_diagnostics(mhd_ctx* ctx, double sums[8], double* max_abs_divb);
  *   "btile"   tile shape of the tile-march y/z B-pair kernel (0 off, 1 = 32x8, 2 = 64x8, 3 = 64x4, 4 = 128x4);
  *             used when "bring" = 0
  *   "btma", "bstages"  TMA variant of the tile march (0 off) and its ring depth (4, 6, 8)
- *   "xpack"   x kernels: 0 scalar mhd_x.cuh | 1 all packed | 2 all lane-pack scalar | 3 packed fluid_x only (default)
+ *   "xpack"   x kernels: 0 scalar mhd_x.cuh | 1 all packed | 2 all one row per thread (default) | 3 packed fluid_x only
  *   "xfuse"   reverse L_x in one kernel: 0 off | 1 fp32 only (default) | 2 always | 3 fp32, packed
  * Unknown keys and out-of-range values return MHD_EINVAL. */
 int mhd_set_option(mhd_ctx* ctx, const char* key, long long value);

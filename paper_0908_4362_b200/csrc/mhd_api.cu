@@ -137,7 +137,7 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_bstages = 6;
   c->opt_pack = 1;
   c->opt_bring = 1;
-  c->opt_xpack = 3;
+  c->opt_xpack = 2;
   c->opt_xfuse = 1;
   c->opt_graph = -1;
   c->sm_count = 148;
@@ -507,7 +507,8 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   constexpr bool f32 = std::is_same<real, float>::value;
   using T2 = typename std::conditional<f32, f2, real>::type;
   // xfuse = 3: the fused operator in packed f2 arithmetic even when the single operators run scalar
-  // xpack = 3: fluid_x packed (1.23 ms at 512^3, scalar 1.29), B pair scalar (0.89 ms, packed 1.14)
+  // measured at 512^3 fp32: fluid_x one row per thread at six blocks per SM 1.21 ms, packed (two rows per thread,
+  // three blocks per SM) 1.23; B pair one row per thread 0.89 ms, packed 1.14: the x kernels want occupancy
   const bool pack = f32 && c->n[1] % 2 == 0 && (c->opt_xpack == 1 || (c->opt_xpack == 3 && kind == 0) || (kind == 2 && c->opt_xfuse == 3));
   const int V = VecOf<real>::V, L = pack ? 2 : 1;
   XArgs<real> A;

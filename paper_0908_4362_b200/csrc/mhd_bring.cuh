@@ -45,7 +45,7 @@ struct BRowRing {
 #define MHD_BRING_MINB 3
 #endif
 #ifndef MHD_BRING_STAGES
-#define MHD_BRING_STAGES 6
+#define MHD_BRING_STAGES 7
 #endif
 // the warp on duty refills a stage that every warp released SLACK+1 steps ago: with no slack the duty
 // warp waits for the slowest warp every step, which couples the warps like a block barrier

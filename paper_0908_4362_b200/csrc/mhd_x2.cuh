@@ -321,7 +321,7 @@ __device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const X
 #define MHD_X2_MINB2 3     // blocks per SM the register budget is cut for, two rows per thread (f2)
 #endif
 #ifndef MHD_X2_MINB1
-#define MHD_X2_MINB1 5     // one row per thread
+#define MHD_X2_MINB1 6     // one row per thread (fluid_x scalar fp32: 80 registers 1.21 ms at 512^3; 5: 96 registers 1.29; 7: spills 1.24)
 #endif
 #ifndef MHD_X2_MINB64
 #define MHD_X2_MINB64 2    // fp64: 256-thread blocks
