@@ -27,20 +27,33 @@ __device__ __forceinline__ double last_lane(double a) { return a; }
 __device__ __forceinline__ float last_lane(float a) { return a; }
 __device__ __forceinline__ float last_lane(f2 a) { return a.v.y; }
 
-// largest c of eq (18) over the lanes of a pack, as the order-preserving bit pattern of mhd_device.cuh.
-// NaN must win the maximum (it poisons dt): compare the bit patterns, not the floats.
-__device__ __forceinline__ unsigned long long pack_speed_bits(const double u[5], double hb2, double gamma) {
+// Largest c of eq (18) over the lanes of a pack, as an order-preserving integer key.  NaN must win the maximum (it
+// poisons dt): compare bit patterns, not floats.  c >= 0 or NaN, and the bit pattern of a non-negative float orders
+// like an unsigned integer with every NaN above +Inf (a NaN with the sign bit set is larger still), so fp32 kernels
+// keep a 32-bit key per thread and widen it to the accumulator's double pattern once, at the end (key_bits).
+__device__ __forceinline__ unsigned long long pack_speed_key(const double u[5], double hb2, double gamma) {
   return speed_bits(cfl_speed_hb2(u, hb2, gamma));
 }
-__device__ __forceinline__ unsigned long long pack_speed_bits(const float u[5], float hb2, float gamma) {
-  return speed_bits(cfl_speed_hb2(u, hb2, gamma));
+__device__ __forceinline__ unsigned int pack_speed_key(const float u[5], float hb2, float gamma) {
+  return __float_as_uint(cfl_speed_hb2(u, hb2, gamma));
 }
-__device__ __forceinline__ unsigned long long pack_speed_bits(const f2 u[5], f2 hb2, float gamma) {
-  const float ua[5] = {u[0].v.x, u[1].v.x, u[2].v.x, u[3].v.x, u[4].v.x};
-  const float ub[5] = {u[0].v.y, u[1].v.y, u[2].v.y, u[3].v.y, u[4].v.y};
-  const unsigned long long ba = speed_bits(cfl_speed_hb2(ua, hb2.v.x, gamma));
-  const unsigned long long bb = speed_bits(cfl_speed_hb2(ub, hb2.v.y, gamma));
-  return ba > bb ? ba : bb;
+// two cells: everything that has a packed form runs packed; rcp, sqrt, |x| and the maxima per lane
+__device__ __forceinline__ unsigned int pack_speed_key(const f2 u[5], f2 hb2, float gamma) {
+  const f2 inv = rcp_(u[0]);
+  const f2 ke = f2(0.5f) * fma_(u[1], u[1], fma_(u[2], u[2], u[3] * u[3])) * inv;
+  const f2 p = f2(gamma - 1.0f) * (u[4] - ke - hb2);
+  const f2 t = fma_(f2(gamma), p, f2(2.0f) * hb2);
+  const float ca = fmaxf(fmaxf(fabsf(u[1].v.x), fabsf(u[2].v.x)), fabsf(u[3].v.x)) * inv.v.x + sqrt_(fabsf(t.v.x) * inv.v.x);
+  const float cb = fmaxf(fmaxf(fabsf(u[1].v.y), fabsf(u[2].v.y)), fabsf(u[3].v.y)) * inv.v.y + sqrt_(fabsf(t.v.y) * inv.v.y);
+  const unsigned int ka = __float_as_uint(ca), kb = __float_as_uint(cb);
+  return ka > kb ? ka : kb;
 }
+__device__ __forceinline__ unsigned long long key_bits(unsigned long long k) { return k; }
+__device__ __forceinline__ unsigned long long key_bits(unsigned int k) { return speed_bits(__uint_as_float(k)); }
+
+// kept for the x kernels: the same as a 64-bit pattern per call
+__device__ __forceinline__ unsigned long long pack_speed_bits(const double u[5], double hb2, double gamma) { return pack_speed_key(u, hb2, gamma); }
+__device__ __forceinline__ unsigned long long pack_speed_bits(const float u[5], float hb2, float gamma) { return key_bits(pack_speed_key(u, hb2, gamma)); }
+__device__ __forceinline__ unsigned long long pack_speed_bits(const f2 u[5], f2 hb2, float gamma) { return key_bits(pack_speed_key(u, hb2, gamma)); }
 
 }  // namespace mhd

@@ -306,14 +306,15 @@ __device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const X
     if (q.live) xstore(A.uo[c], q.o[1], q.o[2], o);
   }
   if (A.cmax_bits) {            // last operator of a step: c of eq (18) from the updated cells (B unchanged by fluid_x)
-    unsigned long long cbest = 0ull;
+    typedef typename PackOf<T>::scalar S;
+    decltype(pack_speed_key((const T*)nullptr, T(), S())) cbest = 0;
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-      const unsigned long long bts = pack_speed_bits(un[v], B[v].hb2, A.gamma);
+      const auto bts = pack_speed_key(un[v], B[v].hb2, (S)A.gamma);
       cbest = bts > cbest ? bts : cbest;
     }
-    cbest = warp_max_u64(q.live ? cbest : 0ull);
-    if ((threadIdx.x & 31) == 0) publish_max(A.cmax_bits, cbest);
+    const unsigned long long cw = warp_max_u64(q.live ? key_bits(cbest) : 0ull);
+    if ((threadIdx.x & 31) == 0) publish_max(A.cmax_bits, cw);
   }
 }
 

@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   FluidPipe<T> pipe;
   pipe.init();
   T bd_lo = ld_pack(A.bd + map_index1(n0 - 3, A.nd, A.bc) * A.sd + base, tag);
-  unsigned long long cbest = 0ull;
+  decltype(pack_speed_key((const T*)nullptr, T(), S())) cbest = 0;
   // During the first three steps the re-reads of u(q-1), u(q-3) return whatever the ring holds: it only
   // feeds warm-up state that is flushed before the first stored cell, like the dummy values of
   // FluidPipe::init().
@@ -151,14 +151,14 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
 #pragma unroll
       for (int k = 0; k < 5; ++k) st_pack(A.uo[k] + off, out[k]);
       if (CM) {                   // last operator of a step: c of eq (18) from the updated cells (B unchanged)
-        const unsigned long long b = pack_speed_bits(out, pipe.hb2_out(), A.gamma);
+        const auto b = pack_speed_key(out, pipe.hb2_out(), (S)A.gamma);
         cbest = b > cbest ? b : cbest;
       }
     }
   }
   if (CM) {
-    cbest = warp_max_u64(cbest);
-    if (lane == 0) publish_max(A.cmax_bits, cbest);
+    const unsigned long long cw = warp_max_u64(key_bits(cbest));
+    if (lane == 0) publish_max(A.cmax_bits, cw);
   }
 }
 
