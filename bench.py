@@ -47,7 +47,7 @@ ALGO_WORDS_STEP = 96          # ideal: each of the six L_i reads 8 fields and wr
 CFL = 0.8
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/r01_c4_step_ncu_full_c.md, profiles/r01_c5_step_ncu_full_b.md); None where no capture exists
-NCU_TRAFFIC = {("c4", "fluid_yz"): 7.058e9, ("c5", "fluid_yz"): 14.10e9}
+NCU_TRAFFIC = {("c4", "fluid_yz"): 7.110e9, ("c5", "fluid_yz"): 14.27e9}    # profiles/r01_c4_step_ncu_full_e.md, r01_c5_step_ncu_full_d.md
 
 
 def peaks():
