@@ -123,6 +123,39 @@ int mhd_get_time(mhd_ctx* ctx, double* t);
  * NULL.  Synchronises. */
 int mhd_diagnostics(mhd_ctx* ctx, double sums[8], double* max_abs_divb);
 
+/* ---- Headless visualisation stage (section 8) --------------------
+ * The paper renders the state where it lives: a vertex buffer for 1-D runs, a pixel buffer with a transfer function
+ * for 2-D runs, a volume renderer for 3-D runs, through OpenGL.  Here the same buffers are plain DEVICE memory owned
+ * by the caller (no graphics API).  The paper gives no formulas, so the mappings are fixed here; all arithmetic is
+ * IEEE fp32, one rounding per operation, in the order written:
+ *   value v   field 0..7: the stored field converted to fp32; MHD_VIZ_PRESSURE (8): with every input converted to
+ *             fp32 first, p = (gamma-1) * ((E - (0.5*((mx*mx + my*my) + mz*mz)) / rho) - 0.5*((bx*bx + by*by) + bz*bz)),
+ *             b = 0.5*(face + next face), next face mapped by the boundary rule
+ *   unit   t = min(max((v - vmin) * inv, 0), 1), inv = fp32(1 / (vmax - vmin)), NaN -> 0;  byte(t) = trunc(t*255 + 0.5)
+ * None of these calls synchronises except mhd_viz_range.  MHD_EINVAL: field out of range, NULL pointer,
+ * vmax <= vmin, index out of range, opacity <= 0; MHD_ENOSTATE before mhd_set_state. */
+enum { MHD_VIZ_PRESSURE = 8 };
+
+/* Smallest and largest finite v over all cells (what a caller passes as vmin, vmax).  Synchronises.
+ * MHD_ENONFINITE if no cell is finite. */
+int mhd_viz_range(mhd_ctx* ctx, int field, double* vmin, double* vmax);
+
+/* 1-D (vertex buffer): for the row (j, k), xy_device[2*i] = -1 + (2*i + 1) * fp32(1/nx), xy_device[2*i+1] = -1 + 2*t;
+ * xy_device: 2*nx floats of device memory. */
+int mhd_viz_curve(mhd_ctx* ctx, int field, int j, int k, double vmin, double vmax, float* xy_device);
+
+/* 2-D (pixel buffer): for the plane k, pixel (i, j) = lut[byte(t)]; lut_rgba_device: 256 RGBA8 entries,
+ * rgba_device: nx*ny RGBA8 pixels, x fastest, both device memory. */
+int mhd_viz_slice(mhd_ctx* ctx, int field, int k, double vmin, double vmax, const unsigned char* lut_rgba_device,
+                  unsigned char* rgba_device);
+
+/* 3-D (volume rendering, orthographic rays along +z, front to back): per pixel (i, j), starting from C = 0, A = 0,
+ * for k = 0 .. nz-1: s = lut[byte(t)], a = min((s.a * fp32(1/255)) * opacity, 1), w = (1 - A) * a,
+ * C.c += w * (s.c * fp32(1/255)) for c = r, g, b, A += w, stop after the sample that makes A >= 0.99.
+ * Pixel = (byte(min(C.r,1)), byte(min(C.g,1)), byte(min(C.b,1)), byte(min(A,1))).  rgba_device: nx*ny RGBA8 pixels. */
+int mhd_viz_volume(mhd_ctx* ctx, int field, double vmin, double vmax, const unsigned char* lut_rgba_device,
+                   double opacity, unsigned char* rgba_device);
+
 /* Tuning knobs, all optional; none changes what is computed beyond rounding order inside the stated tolerances.
  *   "graph"   -1 auto (default: grids of <= 2^22 cells) | 0 | 1: replay whole steps of mhd_step / mhd_run_until
  *             as CUDA graphs (small grids are bound by launch latency)

@@ -50,6 +50,10 @@ SIGNATURES = {
     "mhd_set_step_index": (c_int, [c_void_p, c_longlong]),
     "mhd_get_time": (c_int, [c_void_p, POINTER(c_double)]),
     "mhd_diagnostics": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double)]),
+    "mhd_viz_range": (c_int, [c_void_p, c_int, POINTER(c_double), POINTER(c_double)]),
+    "mhd_viz_curve": (c_int, [c_void_p, c_int, c_int, c_int, c_double, c_double, c_void_p]),
+    "mhd_viz_slice": (c_int, [c_void_p, c_int, c_int, c_double, c_double, c_void_p, c_void_p]),
+    "mhd_viz_volume": (c_int, [c_void_p, c_int, c_double, c_double, c_void_p, c_double, c_void_p]),
     "mhd_set_option": (c_int, [c_void_p, c_char_p, c_longlong]),
     "mhd_launch_count": (c_longlong, [c_void_p]),
     "mhd_last_error": (c_char_p, [c_void_p]),
@@ -69,6 +73,11 @@ mhd_cfl_dt = _lib.mhd_cfl_dt
 mhd_step = _lib.mhd_step
 mhd_step_fixed = _lib.mhd_step_fixed
 mhd_run_until = _lib.mhd_run_until
+mhd_viz_range = _lib.mhd_viz_range
+mhd_viz_curve = _lib.mhd_viz_curve
+mhd_viz_slice = _lib.mhd_viz_slice
+mhd_viz_volume = _lib.mhd_viz_volume
+MHD_VIZ_PRESSURE = 8
 mhd_apply = _lib.mhd_apply
 mhd_get_step_index = _lib.mhd_get_step_index
 mhd_set_step_index = _lib.mhd_set_step_index
@@ -202,6 +211,25 @@ class Solver:
         dv = c_double()
         self._check(mhd_diagnostics(self._h, sums, byref(dv)))
         return list(sums), dv.value
+
+    # ---- headless visualisation stage: device buffers (torch tensors or raw device pointers) in, nothing copied ----
+    @staticmethod
+    def _dev(x):
+        return x.data_ptr() if _is_torch(x) else int(x)
+
+    def viz_range(self, field):
+        lo, hi = c_double(), c_double()
+        self._check(mhd_viz_range(self._h, int(field), byref(lo), byref(hi)))
+        return lo.value, hi.value
+
+    def viz_curve(self, field, j, k, vmin, vmax, xy):
+        self._check(mhd_viz_curve(self._h, int(field), int(j), int(k), float(vmin), float(vmax), self._dev(xy)))
+
+    def viz_slice(self, field, k, vmin, vmax, lut, rgba):
+        self._check(mhd_viz_slice(self._h, int(field), int(k), float(vmin), float(vmax), self._dev(lut), self._dev(rgba)))
+
+    def viz_volume(self, field, vmin, vmax, lut, opacity, rgba):
+        self._check(mhd_viz_volume(self._h, int(field), float(vmin), float(vmax), self._dev(lut), float(opacity), self._dev(rgba)))
 
     def set_option(self, key, value):
         self._check(mhd_set_option(self._h, key.encode(), int(value)))

@@ -18,6 +18,7 @@
 #include "mhd_yz2.cuh"
 #include "mhd_bring.cuh"
 #include "mhd_x2.cuh"
+#include "mhd_viz.cuh"
 
 using namespace mhd;
 
@@ -922,6 +923,97 @@ extern "C" int mhd_diagnostics(mhd_ctx* c, double sums[8], double* max_abs_divb)
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   if (sums) memcpy(sums, h, 8 * sizeof(double));
   if (max_abs_divb) *max_abs_divb = h[8];   // the bit pattern of a non-negative double IS that double
+  return MHD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// headless visualisation stage (section 8; mhd_viz.cuh)
+// ---------------------------------------------------------------------------------------------
+template <class real>
+static VizArgs<real> make_viz(const mhd_ctx* c, int field, double vmin, double vmax) {
+  VizArgs<real> A;
+  for (int f = 0; f < 8; ++f) A.f[f] = (const real*)c->cur[f];
+  A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2]; A.bc = c->bc;
+  A.field = field;
+  A.gamma = (float)c->gamma;
+  A.vmin = (float)vmin;
+  A.inv = (float)(1.0 / (vmax - vmin));
+  return A;
+}
+
+static int viz_check(mhd_ctx* c, int field, const char* who) {
+  if (field < 0 || field > MHD_VIZ_PRESSURE) return fail(c, MHD_EINVAL, "%s: field must be 0..8", who);
+  if (!c->has_state) return fail(c, MHD_ENOSTATE, "%s: no state set", who);
+  return MHD_OK;
+}
+
+static unsigned viz_grid(const mhd_ctx* c, long long items) {
+  const long long want = (items + 255) / 256, cap = (long long)c->sm_count * 8;
+  return (unsigned)(want < cap ? (want > 0 ? want : 1) : cap);
+}
+
+extern "C" int mhd_viz_range(mhd_ctx* c, int field, double* vmin, double* vmax) {
+  if (!c) return MHD_EINVAL;
+  if (!vmin || !vmax) return fail(c, MHD_EINVAL, "mhd_viz_range: NULL output");
+  int rc = viz_check(c, field, "mhd_viz_range");
+  if (rc) return rc;
+  unsigned int* lohi = (unsigned int*)(c->diag + 16);          // scratch inside the scalar block
+  const unsigned int init[2] = {0xffffffffu, 0u};
+  CUDA_TRY(c, cudaMemcpyAsync(lohi, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+  const unsigned grid = viz_grid(c, (long long)c->N);
+  if (c->precision == MHD_F32) viz_range_kernel<float><<<grid, 256, 0, c->stream>>>(make_viz<float>(c, field, 0.0, 1.0), lohi);
+  else viz_range_kernel<double><<<grid, 256, 0, c->stream>>>(make_viz<double>(c, field, 0.0, 1.0), lohi);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  unsigned int h[2];
+  CUDA_TRY(c, cudaMemcpyAsync(h, lohi, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (h[0] > h[1]) return fail(c, MHD_ENONFINITE, "mhd_viz_range: no finite value");
+  auto unkey = [](unsigned int k) { unsigned int b = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k; float v; memcpy(&v, &b, 4); return (double)v; };
+  *vmin = unkey(h[0]);
+  *vmax = unkey(h[1]);
+  return MHD_OK;
+}
+
+extern "C" int mhd_viz_curve(mhd_ctx* c, int field, int j, int k, double vmin, double vmax, float* xy_device) {
+  if (!c) return MHD_EINVAL;
+  int rc = viz_check(c, field, "mhd_viz_curve");
+  if (rc) return rc;
+  if (!xy_device || !(vmax > vmin) || j < 0 || j >= c->n[1] || k < 0 || k >= c->n[2]) return fail(c, MHD_EINVAL, "mhd_viz_curve: bad argument");
+  const float invn = (float)(1.0 / c->n[0]);
+  const unsigned grid = (unsigned)((c->n[0] + 255) / 256);
+  if (c->precision == MHD_F32) viz_curve_kernel<float><<<grid, 256, 0, c->stream>>>(make_viz<float>(c, field, vmin, vmax), j, k, invn, (float2*)xy_device);
+  else viz_curve_kernel<double><<<grid, 256, 0, c->stream>>>(make_viz<double>(c, field, vmin, vmax), j, k, invn, (float2*)xy_device);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return MHD_OK;
+}
+
+extern "C" int mhd_viz_slice(mhd_ctx* c, int field, int k, double vmin, double vmax, const unsigned char* lut_rgba_device,
+                             unsigned char* rgba_device) {
+  if (!c) return MHD_EINVAL;
+  int rc = viz_check(c, field, "mhd_viz_slice");
+  if (rc) return rc;
+  if (!lut_rgba_device || !rgba_device || !(vmax > vmin) || k < 0 || k >= c->n[2]) return fail(c, MHD_EINVAL, "mhd_viz_slice: bad argument");
+  const unsigned grid = viz_grid(c, (long long)c->n[0] * c->n[1]);
+  if (c->precision == MHD_F32) viz_slice_kernel<float><<<grid, 256, 0, c->stream>>>(make_viz<float>(c, field, vmin, vmax), k, (const uchar4*)lut_rgba_device, (uchar4*)rgba_device);
+  else viz_slice_kernel<double><<<grid, 256, 0, c->stream>>>(make_viz<double>(c, field, vmin, vmax), k, (const uchar4*)lut_rgba_device, (uchar4*)rgba_device);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return MHD_OK;
+}
+
+extern "C" int mhd_viz_volume(mhd_ctx* c, int field, double vmin, double vmax, const unsigned char* lut_rgba_device,
+                              double opacity, unsigned char* rgba_device) {
+  if (!c) return MHD_EINVAL;
+  int rc = viz_check(c, field, "mhd_viz_volume");
+  if (rc) return rc;
+  if (!lut_rgba_device || !rgba_device || !(vmax > vmin) || !(opacity > 0.0)) return fail(c, MHD_EINVAL, "mhd_viz_volume: bad argument");
+  const unsigned grid = viz_grid(c, (long long)c->n[0] * c->n[1]);
+  if (c->precision == MHD_F32) viz_volume_kernel<float><<<grid, 256, 0, c->stream>>>(make_viz<float>(c, field, vmin, vmax), (const uchar4*)lut_rgba_device, (float)opacity, (uchar4*)rgba_device);
+  else viz_volume_kernel<double><<<grid, 256, 0, c->stream>>>(make_viz<double>(c, field, vmin, vmax), (const uchar4*)lut_rgba_device, (float)opacity, (uchar4*)rgba_device);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
   return MHD_OK;
 }
 

@@ -455,3 +455,72 @@ def test_second_workload_set_generators():
     assert np.allclose(f3[5] ** 2 + f3[6] ** 2 + f3[7] ** 2, 1.0)
     p3 = (m3["gamma"] - 1.0) * (f3[4] - 0.5)
     assert abs(p3.max() - 10.0) < 1e-12 and abs(p3.min() - 0.1) < 1e-12
+
+
+# ---- visualisation stage (oracle/viz.py; include/mhd.h is the definition, the paper prints none) --------------------
+def _viz_fields(shape, seed):
+    from tests.parity_utils import random_state
+    return random_state(*shape, seed=seed)
+
+
+def test_viz_value_pressure_recovers_the_pressure_the_state_was_built_from():
+    from oracle import viz
+    from paper_0908_4362_b200 import inputs
+    f, meta = inputs.blast2d(64)
+    p = viz.value(f, viz.PRESSURE, meta["gamma"], meta["bc"])
+    assert abs(float(p.max()) - 10.0) < 1e-5 and abs(float(p.min()) - 0.1) < 1e-5
+    f3, m3 = inputs.turbulence(16, 12, 8)                    # p = 1 everywhere by construction
+    p3 = viz.value(f3, viz.PRESSURE, m3["gamma"], m3["bc"])
+    assert np.abs(p3 - 1.0).max() < 2e-5
+    assert viz.value(f3, 0, m3["gamma"], m3["bc"]).dtype == np.float32
+
+
+def test_viz_unit_byte_and_curve_closed_forms():
+    from oracle import viz
+    v = np.array([-1.0, 0.0, 0.25, 0.5, 1.0, 7.0, np.nan], dtype=np.float32)
+    t = viz.unit(v, 0.0, 1.0)
+    assert list(t) == [0.0, 0.0, 0.25, 0.5, 1.0, 1.0, 0.0]
+    assert list(viz.byte(t)) == [0, 0, 64, 128, 255, 255, 0]          # trunc(t*255 + 0.5)
+    nx = 8
+    f = [np.zeros((1, 1, nx)) for _ in range(8)]
+    f[0][0, 0, :] = np.linspace(2.0, 4.0, nx)
+    xy = viz.curve(f, 0, 1.4, 0, 0, 0, 2.0, 4.0)
+    assert xy.shape == (nx, 2)
+    assert np.allclose(xy[:, 0], -1 + (2 * np.arange(nx) + 1) / nx, atol=1e-7)      # cell centres of [-1, 1]
+    assert np.allclose(xy[:, 1], np.linspace(-1.0, 1.0, nx), atol=1e-6)
+    assert viz.value_range(f, 0, 1.4, 0) == (2.0, 4.0)
+
+
+def test_viz_slice_is_a_table_lookup_and_volume_follows_the_compositing_closed_form():
+    from oracle import viz
+    lut = np.zeros((256, 4), dtype=np.uint8)
+    lut[:, 0] = np.arange(256)
+    lut[:, 1] = 255 - np.arange(256)
+    lut[:, 2] = 7
+    lut[:, 3] = 51                                                        # a = 0.2 per sample
+    f = _viz_fields((12, 9, 30), 4)
+    g = 5.0 / 3.0
+    lo, hi = viz.value_range(f, 0, g, 0)
+    img = viz.slice_rgba(f, 0, g, 0, 3, lo, hi, lut)
+    t = (np.asarray(f[0][3], np.float64) - lo) / (hi - lo)
+    assert img.shape == (9, 12, 4) and img.dtype == np.uint8
+    assert np.abs(img[..., 0].astype(int) - np.rint(t * 255)).max() <= 1     # red channel = byte(t), up to fp32 rounding
+    assert np.all(img[..., 0].astype(int) + img[..., 1] == 255) and np.all(img[..., 2] == 7)
+    assert img[..., 0].max() == 255 and img[..., 0].min() == 0
+    # volume: constant colour and opacity a per sample -> A_n = 1 - (1-a)^n, C = A * colour, cut at the first A >= 0.99
+    const = [np.ones((30, 9, 12)) for _ in range(8)]
+    lut2 = np.zeros((256, 4), dtype=np.uint8)
+    lut2[:] = (255, 128, 0, 51)
+    out = viz.volume_rgba(const, 0, g, 0, 0.0, 2.0, lut2, 1.0)
+    n_stop = int(np.ceil(np.log(0.01) / np.log(0.8)))                      # 21 samples reach A >= 0.99
+    A = 1 - 0.8 ** n_stop
+    assert n_stop == 21 and np.all(out[..., 3] == int(A * 255 + 0.5))
+    assert np.all(out[..., 0] == int(A * 255 + 0.5)) and np.all(out[..., 2] == 0)
+    assert np.all(np.abs(out[..., 1].astype(int) - int(A * 128 / 255 * 255 + 0.5)) <= 1)
+    out_thin = viz.volume_rgba(const, 0, g, 0, 0.0, 2.0, lut2, 0.01)       # never terminates early: all 30 samples
+    a = 51 / 255 * 0.01
+    assert np.all(np.abs(out_thin[..., 3].astype(int) - int((1 - (1 - a) ** 30) * 255 + 0.5)) <= 1)
+    # opaque first sample hides everything behind it
+    lut3 = lut.copy(); lut3[:, 3] = 255
+    front = viz.volume_rgba(f, 0, g, 0, lo, hi, lut3, 1.0)
+    assert np.array_equal(front[..., :3], viz.slice_rgba(f, 0, g, 0, 0, lo, hi, lut3)[..., :3]) and np.all(front[..., 3] == 255)
