@@ -70,3 +70,23 @@ def test_blast3d_paper_field_parity(B, prec, n):
     # (the sweep order breaks it at truncation level), so only closeness is checked
     rho = np.asarray(got[0], dtype=np.float64)
     assert np.abs(rho - rho.transpose(2, 0, 1)).max() < 0.05 * rho.max()
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_ring_kernels_are_deterministic(B, prec):
+    """the TMA-ring march kernels have no block barrier: warps drift and the elected producer refills stages out
+    of step with the consumers.  Two runs of the same 12 steps must agree bit for bit (a race would not)."""
+    f, meta = inputs.turbulence(256, 48, 40)
+    dtp = np.float32 if prec == "f32" else np.float64
+    f = [np.ascontiguousarray(a, dtype=dtp) for a in f]
+    outs = []
+    for rep in range(3):
+        s = B.Solver(256, 48, 40, meta["gamma"], prec, meta["bc"])
+        s.set_option("graph", rep % 2)
+        s.set_state(f)
+        s.step(12, 0.8)
+        outs.append(s.get_state())
+        s.close()
+    for other in outs[1:]:
+        for x, y in zip(outs[0], other):
+            assert np.array_equal(x, y)
