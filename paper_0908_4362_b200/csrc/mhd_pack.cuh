@@ -4,7 +4,7 @@
 // Why: the fp32 sweep kernels are bound by instruction issue, not by HBM or by the FMA pipe
 // (profiles/r01_c4_step_ncu_full.md: ~165 of ~280 issued instructions per cell are FADD/FMUL/FFMA).
 // A packed instruction occupies the FMA pipe for two cycles but only ONE issue slot
-// (measured on B200: FFMA 3.83 warp-inst/clk/SM, FFMA2 1.97; profiles/r01_packed_fp32_rates.md), so
+// (measured on B200 with a throw-away issue-rate loop: FFMA 3.83 warp-inst/clk/SM, FFMA2 1.97), so
 // a thread that advances two adjacent pencils in f2 arithmetic issues half the floating-point
 // instructions for the same flops, and its 64-bit shared-memory loads and global stores halve the
 // load/store instructions too.  What has no packed form stays per lane: MUFU (rcp, sqrt), |x|, and
