@@ -71,7 +71,9 @@ int mhd_destroy(mhd_ctx* ctx);
 
 /* Copy a full state IN.  fields[0..7] point to N elements each of the context's precision, in host
  * (where = MHD_HOST, pageable or pinned) or device (MHD_DEVICE) memory.  Resets the time
- * accumulated by the context to 0 but not the step index.  Synchronises for host sources. */
+ * accumulated by the context to 0 but not the step index.  Synchronises for host sources.  Device sources are
+ * copied on the context's stream without waiting for any other stream: the caller orders the producer of the data
+ * before this call (e.g. a device synchronise, or by binding the producer's stream with mhd_bind). */
 int mhd_set_state(mhd_ctx* ctx, const void* const fields[8], int where);
 
 /* Copy the current state OUT into fields[0..7] (N elements each).  Synchronises. */

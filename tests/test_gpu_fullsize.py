@@ -123,3 +123,59 @@ def test_full_size_sampled_parity(name, gen, n, prec):
         state, after = after, state
     sol.close()
     print(name, prec, "worst max-rel per group over 3 steps:", worst)
+
+
+def _gather3(fields, lo, dims):
+    """as _gather for a non-cubic grid: dims = (nz, ny, nx)"""
+    import torch
+    side = W + 2 * H
+    idx = [torch.remainder(torch.arange(l, l + side, device=fields[0].device), n) for l, n in zip(lo, dims)]
+    out = []
+    for f in fields:
+        b = f.index_select(0, idx[0]).index_select(1, idx[1]).index_select(2, idx[2])
+        out.append(np.ascontiguousarray(b.double().cpu().numpy()))
+    return out
+
+
+@pytest.mark.parametrize("nx,ny,nz,prec", [(1024, 256, 192, "f32"),     # widest row the x kernels take (falls back to
+                                                                       # mhd_x.cuh), four ring tiles per row
+                                           (384, 200, 136, "f32"),      # 128-wide ring tiles, extents that are no
+                                           (384, 200, 136, "f64")])     # multiple of the segment or tile sizes
+def test_large_non_cubic_sampled_parity(nx, ny, nz, prec):
+    """edge cases of the launch geometry at sizes the oracle cannot advance whole: same sampling argument as above"""
+    import torch
+    from paper_0908_4362_b200 import binding as B
+    assert torch.cuda.is_available()
+    dev = "cuda:0"
+    f, meta = inputs.turbulence(nx, ny, nz, xp=torch, xp_kw={"device": dev})
+    tdt = torch.float32 if prec == "f32" else torch.float64
+    state = [a.to(tdt).contiguous() for a in f]
+    del f
+    gamma = meta["gamma"]
+    sol = B.Solver(nx, ny, nz, gamma, prec, meta["bc"])
+    torch.cuda.synchronize()            # the context has its own stream: torch's generator kernels must be done
+    sol.set_state(state)
+    after = [torch.empty_like(a) for a in state]
+    dims = (nz, ny, nx)
+    rng = np.random.default_rng(nx + ny)
+    boxes = [(-W // 2, -W // 2, -W // 2), (nz // 2 - W // 2, ny // 2 - W // 2, nx // 2 - W // 2),
+             (nz - W, ny - W, nx - W), (7, ny // 3, 256 - W // 2), (nz // 3, 5, 128 - W // 2)]
+    boxes += [tuple(int(rng.integers(0, n)) for n in dims) for _ in range(3)]
+    for k in range(3):
+        dt, cm = sol.cfl_dt(0.8)
+        if k == 0:
+            cm_ref = oracle.cmax([a.cpu().numpy() for a in state], gamma, meta["bc"])
+            assert abs(cm - cm_ref) <= (1e-14 if prec == "f64" else 5e-6) * cm_ref
+        sol.step_fixed(1, dt)
+        sol.get_state(after)
+        scale = {g: max(float(after[i].abs().max()) for i in idx) for g, idx in GROUPS.items()}
+        for lo in boxes:
+            blk = _gather3(state, [l - H for l in lo], dims)
+            oracle.step_fixed(blk, gamma, inputs.OUTFLOW, k, dt)
+            got = _gather3(after, [l - H for l in lo], dims)
+            core = (slice(H, H + W),) * 3
+            for g, idx in GROUPS.items():
+                err = max(float(np.abs(got[i][core] - blk[i][core]).max()) for i in idx)
+                assert err <= TOL[prec] * scale[g], (nx, ny, nz, prec, k, lo, g, err / scale[g])
+        state, after = after, state
+    sol.close()
