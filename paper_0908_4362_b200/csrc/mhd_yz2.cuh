@@ -28,6 +28,9 @@ namespace mhd {
 #ifndef MHD_YZ2_MINB
 #define MHD_YZ2_MINB 3
 #endif
+#ifndef MHD_YZ2_UNROLL
+#define MHD_YZ2_UNROLL 3      // march steps per unrolled loop body
+#endif
 #ifndef MHD_YZ2_STAGES
 #define MHD_YZ2_STAGES 8
 #endif
@@ -111,7 +114,8 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   // During the first three steps the re-reads of u(q-1), u(q-3) return whatever the ring holds: it only
   // feeds warm-up state that is flushed before the first stored cell, like the dummy values of
   // FluidPipe::init().
-#pragma unroll 3
+  constexpr int UNR = MHD_YZ2_UNROLL;
+#pragma unroll UNR
   for (int it = 0; it < niter; ++it) {
     if (((unsigned)it & (NW - 1)) == (unsigned)warp && it + PF < niter) produce(it + PF);
     const unsigned s = (unsigned)it % D;
