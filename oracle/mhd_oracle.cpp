@@ -17,7 +17,9 @@
 // convergence of linear Alfven / fast / slow eigenmodes to their closed-form solution, Sod tube
 // against the exact Riemann solution (B = 0), Orszag-Tang rotation symmetry, uniform-state fixed
 // point, 1-D replication, cyclic-permutation equivariance, Brio-Wu invariants, constant-velocity
-// linear advection of the scalar B scheme, brute-force NumPy restatement on tiny grids.
+// linear advection of the scalar B scheme, brute-force NumPy restatement on tiny grids, and c_max of
+// eq (18) against hand-computed values (uniform state, one moving cell per velocity component, face
+// pattern whose centred average differs from either face, last cell under both boundary rules).
 // Parity unpinned by the paper: PAPER.md prints no numerical field values (figures only), so no
 // golden values from the paper exist; the pins above are mathematical.
 //

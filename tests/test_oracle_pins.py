@@ -438,6 +438,84 @@ def test_cmax_surfaces_nan():
     assert math.isnan(oracle.cmax(f, meta["gamma"], meta["bc"]))
 
 
+# ---------------------------------------------------------------------------------------------
+# c_max of eq (18), against hand-computed values.  Every state below is built from numbers
+# chosen so that the expected c is a short decimal worked out on paper (the arithmetic is written in the
+# comments, the expected values are literals): c = max(|vx|,|vy|,|vz|) + sqrt(|gamma p + B^2| / rho) with B the
+# cell-centred average of the two faces (reading R4) and p = (gamma-1)(E - rho v^2/2 - B^2/2).
+# ---------------------------------------------------------------------------------------------
+def _const_state(shape, rho, v, E, B):
+    nz, ny, nx = shape
+    full = lambda x: np.full((nz, ny, nx), float(x))
+    return [full(rho), full(rho * v[0]), full(rho * v[1]), full(rho * v[2]), full(E), full(B[0]), full(B[1]), full(B[2])]
+
+
+@pytest.mark.parametrize("bc", [P, O])
+@pytest.mark.parametrize("perm", [(0, 1, 2), (1, 2, 0), (2, 0, 1)])
+def test_cmax_uniform_state_hand_computed(bc, perm):
+    # rho = 4, gamma = 5/3, v = (0.3, -0.7, 0.2) (permuted), B = (1, 2, 2) (permuted): B^2 = 9, v^2 = 0.62.
+    # p = 4.2  ->  gamma p = 7,  gamma p + B^2 = 16,  /rho = 4,  sqrt = 2;  max|v| = 0.7  ->  c = 2.7
+    # E = p/(gamma-1) + rho v^2/2 + B^2/2 = 6.3 + 1.24 + 4.5 = 12.04
+    v0, B0 = (0.3, -0.7, 0.2), (1.0, 2.0, 2.0)
+    v = [v0[perm[i]] for i in range(3)]
+    B = [B0[perm[i]] for i in range(3)]
+    f = _const_state((3, 4, 5), 4.0, v, 12.04, B)
+    assert abs(oracle.cmax(f, 5.0 / 3.0, bc) - 2.7) < 1e-14
+    # the largest |v| must come from whichever component holds it: dropping a component from the max would give
+    # 0.3 + 2 = 2.3 for one of the three permutations
+
+
+@pytest.mark.parametrize("comp", [1, 2, 3])
+def test_cmax_picks_the_one_cell_and_the_one_velocity_component(comp):
+    # background at rest: rho = 1, gamma = 2, B = 0, E = 2  ->  p = 2, c = sqrt(4) = 2.
+    # one cell moves with v = -3 along `comp` only: E = 2 + rho v^2/2 = 6.5 keeps p = 2  ->  c = 3 + 2 = 5
+    f = _const_state((4, 3, 6), 1.0, (0, 0, 0), 2.0, (0, 0, 0))
+    assert abs(oracle.cmax(f, 2.0, P) - 2.0) < 1e-15
+    f[comp][2, 1, 4] = -3.0
+    f[4][2, 1, 4] = 6.5
+    assert abs(oracle.cmax(f, 2.0, P) - 5.0) < 1e-15
+    assert abs(oracle.cmax(f, 2.0, O) - 5.0) < 1e-15
+
+
+def test_cmax_uses_the_cell_centred_average_of_the_two_faces():
+    # gamma = 3, rho = 1, v = 0:  c^2 = 3 p + B^2 = 3 * 2 (E - B^2/2) + B^2 = 6 E - 2 B^2  (gamma = 2 would hide B in c).
+    # E = 3; the component along the axis alternates 2, 0 from face to face, so every cell-centred value is 1:
+    #   centre (B = 1): c^2 = 18 - 2 = 16, c = 4.   A face value instead of the average gives B = 2: c^2 = 10, or B = 0: 18.
+    pattern = [2, 0, 2, 0, 2, 0, 2, 0]
+    for axis in range(3):                       # Bx on x-faces, By on y-faces, Bz on z-faces
+        shape = [1, 1, 1]
+        shape[2 - axis] = 8
+        f = _const_state(tuple(shape), 1.0, (0, 0, 0), 3.0, (0, 0, 0))
+        f[5 + axis].ravel()[:] = pattern
+        assert abs(oracle.cmax(f, 3.0, P) - 4.0) < 1e-15
+    # By varies along y only; averaging it along x instead (a transposed operand) would see equal neighbours,
+    # B = 2 or 0, and return sqrt 18
+    k = _const_state((1, 8, 2), 1.0, (0, 0, 0), 3.0, (0, 0, 0))
+    k[6][0, :, :] = np.array(pattern)[:, None]
+    assert abs(oracle.cmax(k, 3.0, P) - 4.0) < 1e-15
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_cmax_last_cell_follows_the_boundary_rule(axis):
+    # gamma = 3, rho = 1, v = 0, E = 9:  c^2 = 6 E - 2 B_c^2 = 54 - 2 B_c^2  (see the test above).
+    # Faces along `axis`: B = 5, 4, 3, 1.  Centres of cells 0..2: 4.5, 3.5, 2  ->  c^2 = 13.5, 29.5, 46.
+    # Last cell (reading R9): periodic wraps to face 0: (1 + 5)/2 = 3 -> c^2 = 36, so the maximum is 46 (cell 2);
+    #                         outflow clamps to its own face: (1 + 1)/2 = 1 -> c^2 = 52, the maximum.
+    shape = [1, 1, 1]
+    shape[2 - axis] = 4
+    f = _const_state(tuple(shape), 1.0, (0, 0, 0), 9.0, (0, 0, 0))
+    f[5 + axis].ravel()[:] = [5, 4, 3, 1]
+    assert abs(oracle.cmax(f, 3.0, P) - math.sqrt(46.0)) < 1e-14
+    assert abs(oracle.cmax(f, 3.0, O) - math.sqrt(52.0)) < 1e-14
+
+
+def test_cmax_negative_pressure_takes_the_absolute_value():
+    # reading R3: c = |v| + sqrt(|gamma p + B^2| / rho).  rho = 2, gamma = 2, v = 0, B = 0, E = -4: p = -4,
+    # gamma p + B^2 = -8, |.|/rho = 4, c = 2 (never NaN for rho > 0)
+    f = _const_state((2, 2, 2), 2.0, (0, 0, 0), -4.0, (0, 0, 0))
+    assert abs(oracle.cmax(f, 2.0, P) - 2.0) < 1e-15
+
+
 def test_second_workload_set_generators():
     """initial data of the paper's E4 / E6: uniform B (div B = 0
     exactly), v = 0, p jump 10 / 0.1 at r = 0.1, and the oracle keeps the 2-D run 2-D"""
