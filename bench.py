@@ -45,9 +45,19 @@ def _gen(inputs, gen, n, **kw):
     return inputs.blast3d(n, paper_field=(gen == "blast3d_paper"), **kw)
 ALGO_WORDS_STEP = 96          # ideal: each of the six L_i reads 8 fields and writes 8
 CFL = 0.8
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
-# captures (profiles/r01_c4_step_ncu_full_c.md, profiles/r01_c5_step_ncu_full_b.md); None where no capture exists
-NCU_TRAFFIC = {("c4", "fluid_yz"): 7.110e9, ("c5", "fluid_yz"): 14.27e9}    # profiles/r01_c4_step_ncu_full_e.md, r01_c5_step_ncu_full_d.md
+SPEC_PEAK_GBS = 8000.0        # the data-sheet HBM3e figure north_star words its target on (context; the roofline uses the measured copy rate)
+# configs' own step counts (BASELINE.json): the headline line is timed at --steps, `long_run` repeats it at these
+CONFIG_STEPS = {"c4": 100, "c5": 50, "c3": 200}
+
+
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed post-processing of the
+    ncu --set full capture (profiles/r02_traffic.json names the capture it came from); None where no capture exists"""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    try:
+        return json.load(open(p))["traffic_bytes_per_launch"][workload][kernel]
+    except Exception:
+        return None
 
 
 def peaks():
@@ -113,10 +123,28 @@ def make_state(gen, n, prec, device):
     return out, meta
 
 
-def oracle_rate(gen, prec, budget_s=12.0, n=96):
+def l2_note(state_bytes):
+    """how the timed state compares with the 126 MB L2 (timing rule: inputs larger than L2, or say so)"""
+    gb = state_bytes / 1e9
+    if state_bytes > 4 * 126e6:
+        return f"state {gb:.2f} GB per copy >> 126 MB L2 (inputs larger than L2, no flush needed)"
+    return f"state {gb:.3f} GB per copy is NOT large against the 126 MB L2: partly L2-resident, not an HBM data point"
+
+
+def oracle_rate(gen, prec, budget_s=12.0, n=96, threads=None):
     """the oracle as it stands, timed on the host cores on a bounded sample of the workload"""
     import oracle
     from paper_0908_4362_b200 import inputs
+    n_all = oracle.num_threads()
+    if threads:
+        oracle.set_num_threads(threads)
+    try:
+        return _oracle_rate(oracle, inputs, gen, prec, budget_s, n)
+    finally:
+        oracle.set_num_threads(n_all)
+
+
+def _oracle_rate(oracle, inputs, gen, prec, budget_s, n):
     f, meta = _gen(inputs, gen, n)
     dt = np.float32 if prec == "f32" else np.float64
     st = [np.array(a, dtype=dt) for a in f]
@@ -172,6 +200,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-breakdown", action="store_true")
+    ap.add_argument("--no-long-run", action="store_true", help="skip the second timed run at the config's own step count")
+    ap.add_argument("--no-others", action="store_true", help="skip the short fp64 (c5) and 256^3 (c3) legs")
     ap.add_argument("--e2e-contexts", type=int, default=2, help="independent contexts pipelining the end-to-end jobs")
     ap.add_argument("--option", action="append", default=[], help="key=value passed to mhd_set_option")
     args = ap.parse_args()
@@ -208,29 +238,43 @@ def main():
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
     # ---- device-resident throughput -----------------------------------------------------------
+    def timed(sl, strm, steps):
+        """steps of mhd_step between two CUDA events on the context's stream; clocks sampled during the region"""
+        with torch.cuda.stream(strm):
+            sampler = ClockSampler(local_rank)
+            sampler.start()
+            time.sleep(0.15)
+            barrier()
+            l0 = sl.launch_count()
+            e0, e1 = ev(), ev()
+            w0 = time.time()
+            e0.record(strm)
+            sl.step(steps, CFL, sync=False)
+            e1.record(strm)
+            barrier()
+            w1 = time.time()
+            l1 = sl.launch_count()
+        return rep.max_over_ranks(e0.elapsed_time(e1)), sampler.stop(w0, w1), int(l1 - l0)
+
     with torch.cuda.stream(stream):
         sol.step(args.warmup, CFL, sync=True)
-        sampler = ClockSampler(local_rank)
-        sampler.start()
-        time.sleep(0.15)
-        barrier()
-        l0 = sol.launch_count()
-        e0, e1 = ev(), ev()
-        w0 = time.time()
-        e0.record(stream)
-        sol.step(args.steps, CFL, sync=False)
-        e1.record(stream)
-        barrier()
-        w1 = time.time()
-        l1 = sol.launch_count()
-    ms = e0.elapsed_time(e1)
-    clocks = sampler.stop(w0, w1)
-    ms = rep.max_over_ranks(ms)
+    ms, clocks, launches = timed(sol, stream, args.steps)
     t_now = sol.time()        # also surfaces a poisoned state
     value = N * world * args.steps / (ms * 1e-3)
+    peak, peak_src = peaks()
+    step_bytes = ALGO_WORDS_STEP * esize
+
+    # the same at the config's own step count (BASELINE.json: c4 100 steps): long runs sit under the 1000 W power cap
+    long_run = None
+    ksteps = CONFIG_STEPS.get(args.workload)
+    if ksteps and ksteps != args.steps and not args.no_long_run:
+        lms, lclocks, _ = timed(sol, stream, ksteps)
+        lval = N * world * ksteps / (lms * 1e-3)
+        long_run = {"steps": ksteps, "ms_per_step": lms / ksteps, "value": lval, "clocks": lclocks,
+                    "roofline_step_frac": step_bytes * (lval / world) / 1e9 / peak,
+                    "roofline_step_frac_of_spec_peak": step_bytes * (lval / world) / 1e9 / SPEC_PEAK_GBS}
 
     # ---- per-kernel breakdown and roofline of the dominant kernel (rank 0) ---------------------
-    peak, peak_src = peaks()
     roofline, breakdown = None, None
     if rank == 0 and not args.no_breakdown:
         dtv, _ = sol.cfl_dt(CFL)
@@ -251,6 +295,10 @@ def main():
                 torch.cuda.synchronize()
                 kms = a.elapsed_time(b) / reps                 # includes the 1-thread set_dt launch (~2 us)
                 breakdown[name] = {"ms": kms, "algo_GBps": words * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": words}
+            # the stand-alone c_max pass (first step / after mhd_apply only; steps fuse it into their last kernel):
+            # cmax_reuse = 0 makes every mhd_cfl_dt run the reduction instead of returning the cached c_max
+            sol.set_option("cmax_reuse", 0)
+            sol.cfl_dt(CFL)
             a, b = ev(), ev()
             torch.cuda.synchronize()
             a.record(stream)
@@ -258,7 +306,8 @@ def main():
                 sol.cfl_dt(CFL)
             b.record(stream)
             torch.cuda.synchronize()
-            kms = a.elapsed_time(b) / reps
+            sol.set_option("cmax_reuse", 1)
+            kms = a.elapsed_time(b) / reps             # includes the D2H read of dt and its synchronisation
             breakdown["cfl"] = {"ms": kms, "algo_GBps": 8 * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": 8}
         # Dominant kernel = largest share of a step.  Launches per step, averaged over the three sweep orders:
         # fluid_y, fluid_z 2 each (one kernel template, fluid_yz_ring_kernel, 4 launches), B pair y/z 2 each
@@ -275,12 +324,14 @@ def main():
             kms, words = breakdown[dom]["ms"], breakdown[dom]["words_per_cell"]
         ach = words * esize * N / (kms * 1e-3) / 1e9
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
+                    "traffic": ncu_traffic(args.workload, dom), "peak_source": peak_src,
+                    "frac_of_spec_peak": ach / SPEC_PEAK_GBS,
                     "algorithmic_bytes_per_launch": words * esize * N, "ms_per_launch": kms,
                     "share_of_step": share[dom] / sum(share.values()),
                     "step": {"algorithmic_bytes_per_cell_step": ALGO_WORDS_STEP * esize,
                              "achieved": ALGO_WORDS_STEP * esize * (value / world) / 1e9,
-                             "frac": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / peak}}
+                             "frac": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / peak,
+                             "frac_of_spec_peak": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / SPEC_PEAK_GBS}}
 
     # ---- end to end through the C ABI with HOST buffers ----------------------------------------
     e2e = None
@@ -337,10 +388,44 @@ def main():
             s2.close()
         del hosts
 
+    # ---- the other bandwidth-bound configs, short legs: c5 (512^3 fp64) and c3 (256^3 fp32 blast) -------------
+    # BASELINE.json's metric is "fp32 & fp64 at 256^3/512^3": the headline line is c4; these make the rest driver-measured
+    others = None
+    if world == 1 and args.workload == "c4" and not args.no_others:
+        sol.close()
+        sol = None
+        del ws, state
+        torch.cuda.empty_cache()
+        others = {}
+        for name, ksteps in (("c5", 10), ("c3", 50)):
+            g2, n2, p2, d2 = WORKLOADS[name]
+            st2, m2 = make_state(g2, n2, p2, device)
+            ws2 = torch.empty(B.mhd_workspace_bytes(n2, n2, n2, B.MHD_F32 if p2 == "f32" else B.MHD_F64), dtype=torch.uint8, device=device)
+            s2 = B.Solver(n2, n2, n2, m2["gamma"], p2, m2["bc"], workspace=ws2, stream=stream)
+            torch.cuda.synchronize()
+            s2.set_state(st2)
+            with torch.cuda.stream(stream):
+                s2.step(args.warmup, CFL, sync=True)
+            oms, oclk, _ = timed(s2, stream, ksteps)
+            s2.time()
+            oval = n2 ** 3 * ksteps / (oms * 1e-3)
+            es2 = 4 if p2 == "f32" else 8
+            others[name] = {"workload": d2, "dtype": p2, "steps": ksteps, "ms_per_step": oms / ksteps, "value": oval,
+                            "unit": "cell-updates/s", "clocks": oclk,
+                            "roofline_step_frac": ALGO_WORDS_STEP * es2 * oval / 1e9 / peak,
+                            "roofline_step_frac_of_spec_peak": ALGO_WORDS_STEP * es2 * oval / 1e9 / SPEC_PEAK_GBS,
+                            "l2": l2_note(8 * n2 ** 3 * es2)}
+            s2.close()
+            del s2, ws2, st2
+            torch.cuda.empty_cache()
+
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
         v, cores, sample = oracle_rate(gen, prec)
         cpu = {"value": v, "unit": "cell-updates/s", "cores": cores, "kind": "oracle", "sample": sample}
+        # the baseline of record (the paper's own CPU comparison is a serial code on one core)
+        v1, c1, sample1 = oracle_rate(gen, prec, budget_s=6.0, threads=1)
+        cpu["serial"] = {"value": v1, "unit": "cell-updates/s", "cores": c1, "kind": "oracle", "sample": sample1}
 
     if rank == 0:
         out = {
@@ -350,13 +435,14 @@ def main():
             "dtype": prec, "data": "synthetic",
             "config": {"workload": f"{args.workload}: {desc}", "grid": [n, n, n], "cfl": CFL, "gamma": meta["gamma"],
                        "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "l2": f"state {8 * N * esize / 1e9:.2f} GB per copy >> 126 MB L2 (inputs larger than L2, no flush needed)",
+                       "l2": l2_note(8 * N * esize),
                        "t_grid_after": t_now},
-            "clocks": clocks, "gpu_launches": int(l1 - l0), "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+            "clocks": clocks, "gpu_launches": launches, "long_run": long_run, "others": others, "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
             "kernels": breakdown,
         }
         print(json.dumps(out))
-    sol.close()
+    if sol is not None:
+        sol.close()
     rep.close()
 
 

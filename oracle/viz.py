@@ -56,7 +56,7 @@ def byte(t):
 
 def value_range(fields, field, gamma, bc):
     v = value(fields, field, gamma, bc)
-    v = v[np.isfinite(v) | np.isinf(v)]                       # NaN cells are skipped
+    v = v[np.isfinite(v)]                                     # NaN and +-Inf cells are skipped (mhd.h: finite values)
     return float(v.min()), float(v.max())
 
 

@@ -62,6 +62,7 @@ struct mhd_ctx {
   long long launches;
   // options
   int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages, opt_pack, opt_bring, opt_xpack, opt_xfuse;
+  int opt_cmax_reuse;      // 1: mhd_cfl_dt returns the cached c_max when the state has not changed; 0: always reduce
   int opt_graph;           // -1 auto (small grids), 0 never, 1 always: replay whole steps as CUDA graphs
   StepGraph graphs[64];    // one per (step index mod 3, reduction flags, clip)
   int sm_count;
@@ -141,6 +142,7 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_xpack = 2;
   c->opt_xfuse = 1;
   c->opt_graph = -1;
+  c->opt_cmax_reuse = 1;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -224,7 +226,8 @@ extern "C" int mhd_set_state(mhd_ctx* c, const void* const fields[8], int where)
   const cudaMemcpyKind kind = where == MHD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
   for (int f = 0; f < 8; ++f) CUDA_TRY(c, cudaMemcpyAsync(c->cur[f], fields[f], c->N * c->esize, kind, c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->sc, 0, sizeof(Scalars), c->stream));
-  if (where == MHD_HOST) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  // the caller's pointers need not outlive the call (mhd.h): wait for the copies, device sources included
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   c->has_state = true;
   c->acc_valid = c->fin_valid = false;
   return MHD_OK;
@@ -708,7 +711,7 @@ static int read_scalars(mhd_ctx* c, Scalars* h) {
 // make sc->cmax / sc->dt current: run the reduction only if no fused one is pending
 static int refresh_dt(mhd_ctx* c, double cfl, int advance, int clip = 0) {
   int reuse = 0;
-  if (c->fin_valid) reuse = 1;
+  if (c->fin_valid && (c->opt_cmax_reuse || advance)) reuse = 1;
   else if (!c->acc_valid) {
     int rc = arm_accumulator(c);
     if (rc) return rc;
@@ -725,6 +728,9 @@ static int refresh_dt(mhd_ctx* c, double cfl, int advance, int clip = 0) {
 }
 
 static bool graphs_wanted(const mhd_ctx* c) {
+  // stream capture is not permitted on the legacy default stream (mhd_bind with a NULL stream) nor on the
+  // per-thread default stream: launch the kernels directly there
+  if (c->stream == nullptr || c->stream == cudaStreamLegacy || c->stream == cudaStreamPerThread) return false;
   if (c->opt_graph >= 0) return c->opt_graph != 0;
   return c->N <= ((size_t)1 << 22);
 }
@@ -1033,6 +1039,7 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   if (!strcmp(key, "pack")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "pack must be 0, 1, 128 or 256"); c->opt_pack = (int)value; return MHD_OK; }
   if (!strcmp(key, "xpack")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 0..3"); c->opt_xpack = (int)value; return MHD_OK; }
   if (!strcmp(key, "xfuse")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xfuse must be 0, 1 (fp32 only), 2 (always) or 3 (fp32, packed)"); c->opt_xfuse = (int)value; return MHD_OK; }
+  if (!strcmp(key, "cmax_reuse")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "cmax_reuse must be 0 or 1"); c->opt_cmax_reuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "graph")) { if (value < -1 || value > 1) return fail(c, MHD_EINVAL, "graph must be -1 (auto), 0 or 1"); c->opt_graph = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }
   return fail(c, MHD_EINVAL, "unknown option '%s'", key);

@@ -30,38 +30,46 @@ __device__ __forceinline__ int map_index1(int q, int n, int bc) {
   return q < 0 ? 0 : (q >= n ? n - 1 : q);
 }
 
+// MHD_F32_IEEE (diagnostic builds only, R15): IEEE division and square root and no fused multiply-add in
+// fp32, to measure how much of the fp32 distance to the oracle comes from MUFU and contraction (answer: none of it).
+#ifndef MHD_F32_IEEE
 __device__ __forceinline__ float rcp_(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#else
+__device__ __forceinline__ float rcp_(float x) { return __fdiv_rn(1.0f, x); }
+#endif
 #ifndef MHD_F64_IEEE_DIV
-// fp64: MUFU.RCP64H seed (about 20 bits) + two Newton steps: relative error a few 1e-16, no slow path and no
-// range check, half the dependent DFMA chain of IEEE division.  The fp64 kernels are bound by the latency of
-// exactly these chains (profiles/r01_c5_step_ncu_full.md), and the 1e-12 per-step tolerance leaves ~10^4 ulp.
-// x = 0 or denormal gives NaN, which only ever reaches a discarded select operand (vl_full with a*b <= 0).
+// fp64: MUFU.RCP64H seed (relative error e <= 2^-23) + ONE third-order step  r (1 + e + e^2),  e = 1 - x r:  error e^3
+// = 2^-69, three dependent DFMAs, no slow path and no range check (IEEE division: ~10 DFMAs plus a slow path; two
+// Newton steps: four).  The fp64 kernels are bound by the FP64 pipe and by the latency of exactly these chains
+// (profiles/r01_c5_step_ncu_full_d.md).  x = 0 or denormal gives NaN, which only ever reaches a discarded select
+// operand (vl_full with a*b <= 0).
 __device__ __forceinline__ double rcp_(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  return fma(r, e, r);
+  const double e = fma(-x, r, 1.0);
+  const double e2 = fma(e, e, e);
+  return fma(r, e2, r);
 }
 #else
 __device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
 #endif
+#ifndef MHD_F32_IEEE
 __device__ __forceinline__ float sqrt_(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#else
+__device__ __forceinline__ float sqrt_(float x) { return __fsqrt_rn(x); }
+#endif
 #ifndef MHD_F64_IEEE_DIV
-// fp64 square root of x >= 0: MUFU.RSQ64H seed, two coupled Newton (Goldschmidt) steps on g ~ sqrt(x), h ~ 1/(2 sqrt(x))
-// and one residual correction; relative error a few 1e-16.
+// fp64 square root of x >= 0: MUFU.RSQ64H seed y (relative error <= 2^-23), one third-order step on the reciprocal
+// root  y (1 + e/2 + 3 e^2/8),  e = 1 - x y^2  (error ~ e^3), then sqrt = x y: six dependent operations, result within
+// an ulp or two (the 1e-12 per-step tolerance leaves 10^4).
 __device__ __forceinline__ double sqrt_(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double g = x * y, h = 0.5 * y;
-  double r = fma(-g, h, 0.5);
-  g = fma(g, r, g); h = fma(h, r, h);
-  r = fma(-g, h, 0.5);
-  g = fma(g, r, g); h = fma(h, r, h);
-  const double d = fma(-g, g, x);
-  g = fma(d, h, g);
-  return x > 0.0 ? g : 0.0;
+  const double t = x * y;
+  const double e = fma(-t, y, 1.0);
+  const double p = fma(0.375, e, 0.5) * e;
+  y = fma(y, p, y);
+  return x > 0.0 ? x * y : 0.0;
 }
 #else
 __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
@@ -70,9 +78,17 @@ __device__ __forceinline__ float abs_(float x) { return fabsf(x); }
 __device__ __forceinline__ double abs_(double x) { return fabs(x); }
 // a*b + c and c - a*b as one rounding (the scalar forms are what nvcc's contraction produces anyway;
 // they are spelled out so that the packed type f2 of mhd_pack.cuh gets FFMA2 in the same places)
+#ifndef MHD_F32_IEEE
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+#else
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fadd_rn(__fmul_rn(a, b), c); }
+#endif
 __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+#ifndef MHD_F32_IEEE
 __device__ __forceinline__ float fnma_(float a, float b, float c) { return fmaf(-a, b, c); }
+#else
+__device__ __forceinline__ float fnma_(float a, float b, float c) { return __fadd_rn(__fmul_rn(-a, b), c); }
+#endif
 __device__ __forceinline__ double fnma_(double a, double b, double c) { return fma(-a, b, c); }
 // the two discrete switches of the scheme (reading R8: strict > 0)
 __device__ __forceinline__ float pos_or_zero(float s, float r) { return s > 0.0f ? r : 0.0f; }

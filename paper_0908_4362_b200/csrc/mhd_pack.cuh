@@ -32,8 +32,13 @@ __device__ __forceinline__ f2 operator-(f2 a) { return f2(-a.v.x, -a.v.y); }    
 __device__ __forceinline__ f2 operator+(f2 a, f2 b) { return f2(__fadd2_rn(a.v, b.v)); }
 __device__ __forceinline__ f2 operator-(f2 a, f2 b) { return f2(__fadd2_rn(a.v, (-b).v)); }
 __device__ __forceinline__ f2 operator*(f2 a, f2 b) { return f2(__fmul2_rn(a.v, b.v)); }
+#ifndef MHD_F32_IEEE
 __device__ __forceinline__ f2 fma_(f2 a, f2 b, f2 c) { return f2(__ffma2_rn(a.v, b.v, c.v)); }
 __device__ __forceinline__ f2 fnma_(f2 a, f2 b, f2 c) { return f2(__ffma2_rn((-a).v, b.v, c.v)); }
+#else
+__device__ __forceinline__ f2 fma_(f2 a, f2 b, f2 c) { return f2(__fadd2_rn(__fmul2_rn(a.v, b.v), c.v)); }
+__device__ __forceinline__ f2 fnma_(f2 a, f2 b, f2 c) { return f2(__fadd2_rn(__fmul2_rn((-a).v, b.v), c.v)); }
+#endif
 
 // per-lane operations (no packed form in the ISA)
 __device__ __forceinline__ float rcp_(float x);

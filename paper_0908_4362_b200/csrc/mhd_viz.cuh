@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(256) viz_range_kernel(const VizArgs<real> A, u
   for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < N; idx += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(idx % A.nx), j = (int)((idx / A.nx) % A.ny), k = (int)(idx / sz);
     const float v = viz_value(A, i, j, k);
-    if (v == v) {
+    if (isfinite(v)) {                 // NaN and +-Inf cells are skipped (mhd.h: smallest and largest FINITE value)
       const unsigned int key = viz_key(v);
       lo = key < lo ? key : lo;
       hi = key > hi ? key : hi;

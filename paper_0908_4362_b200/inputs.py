@@ -126,13 +126,15 @@ def orszag_tang(n=256, nz=1):
 # ----------------------------------------------------------------------------------------------
 # config 3: 3-D blast wave (BASELINE.json configs[2]; PAPER.md:539-559 for rho, p, r, gamma)
 # ----------------------------------------------------------------------------------------------
-def blast3d(n=256, xp=np, xp_kw=None, paper_field=False):
+def blast3d(n=256, xp=np, xp_kw=None, paper_field=False, centre=(0.0, 0.0, 0.0)):
     """paper_field=True: the paper's own experiment E6, B = (1,1,1)/sqrt(3) instead of
-    BASELINE.json's (1,1,0)/sqrt(2); same rho, p, radius"""
+    BASELINE.json's (1,1,0)/sqrt(2); same rho, p, radius.
+    centre = (x, y, z) of the high-pressure sphere (default: the origin, as BASELINE.json configs[2] has it; an
+    off-grid centre removes the mirror symmetry of the discrete data, R15)"""
     xp_kw = xp_kw or {}
     gamma = 5.0 / 3.0
     c = (xp.arange(n, dtype=xp.float64, **xp_kw) + 0.5) / n - 0.5
-    r2 = c[None, None, :] ** 2 + c[None, :, None] ** 2 + c[:, None, None] ** 2
+    r2 = (c[None, None, :] - centre[0]) ** 2 + (c[None, :, None] - centre[1]) ** 2 + (c[:, None, None] - centre[2]) ** 2
     shape = (n, n, n)
     one = xp.ones(shape, dtype=xp.float64, **xp_kw)
     p = xp.where(r2 < 0.1 * 0.1, 10.0 * one, 0.1 * one)

@@ -16,7 +16,7 @@ import pytest
 
 import oracle
 from paper_0908_4362_b200 import inputs
-from tests.parity_utils import GROUPS
+from tests.parity_utils import GROUPS, fp32_step_gate
 
 pytestmark = pytest.mark.gpu
 
@@ -98,28 +98,20 @@ def test_full_size_sampled_parity(name, gen, n, prec):
         scale = {g: max(float(after[i].abs().max()) for i in idx) for g, idx in GROUPS.items()}
         for lo in _boxes(name, n, rng):
             blk = _gather(state, [l - H for l in lo], n)
-            oracle.step_fixed(blk, gamma, inputs.OUTFLOW, k, dt)
             got = _gather(after, [l - H for l in lo], n)
             core = (slice(H, H + W),) * 3
-            blk32 = None
+            if prec == "f32":           # plain 1e-5, or the tie-aware gate of tests/parity_utils.py where the oracle itself is that sensitive
+                errs = fp32_step_gate(got, blk, gamma, inputs.OUTFLOW, k, dt, core=core, scale=scale, tol=TOL[prec], tag=f"{name} box {lo}")
+                if name != "c3":        # smooth data: no exact ties, the plain tolerance holds everywhere
+                    assert max(errs.values()) <= TOL[prec], (name, k, lo, errs)
+                for g in GROUPS:
+                    worst[g] = max(worst[g], errs[g])
+                continue
+            oracle.step_fixed(blk, gamma, inputs.OUTFLOW, k, dt)
             for g, idx in GROUPS.items():
                 err = max(float(np.abs(got[i][core] - blk[i][core]).max()) for i in idx)
                 worst[g] = max(worst[g], err / scale[g])
-                if err <= TOL[prec] * scale[g]:
-                    continue
-                # fp32 only (R15): at a strong discontinuity the scheme's discrete switches
-                # (a*b > 0, vh > 0) sit on rounding noise, and fp32 rounding ALONE moves isolated cells by
-                # more than 1e-5 (oracle<float> against oracle<double> on the 96^3 blast: 3.6e-5 in B at the
-                # second step).  There the yardstick is that spread, measured on this very block by the
-                # oracle in both precisions, plus an L1 bound that a wrong kernel cannot meet.
-                assert prec == "f32", (name, k, lo, g, err / scale[g])
-                if blk32 is None:
-                    blk32 = [np.ascontiguousarray(a, dtype=np.float32) for a in _gather(state, [l - H for l in lo], n)]
-                    oracle.step_fixed(blk32, gamma, inputs.OUTFLOW, k, dt)
-                spread = max(float(np.abs(blk32[i][core].astype(np.float64) - blk[i][core]).max()) for i in idx)
-                l1 = sum(float(np.abs(got[i][core] - blk[i][core]).sum()) for i in idx) / (len(idx) * W ** 3)
-                assert err <= 3.0 * spread + TOL[prec] * scale[g], (name, k, lo, g, err / scale[g], spread / scale[g])
-                assert l1 <= 1e-6 * scale[g], (name, k, lo, g, l1 / scale[g])
+                assert err <= TOL[prec] * scale[g], (name, k, lo, g, err / scale[g])
         state, after = after, state
     sol.close()
     print(name, prec, "worst max-rel per group over 3 steps:", worst)

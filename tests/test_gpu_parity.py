@@ -218,6 +218,26 @@ def test_fp32_l1_after_100_steps_3d(B):
     assert worst(e) <= TOL32_L1_100, e
 
 
+@pytest.mark.parametrize("name", ["c3", "c4"])
+def test_fp32_l1_after_100_steps_at_128_cubed(B, name):
+    """north_star: 1e-3 L1 after 100 steps in fp32.  SURVEY.md 8(d): where the full size is too slow for the oracle, the
+    same config at 128^3 for the full step count: c3 (blast wave: shocks) and c4 (turbulence-like state),
+    the oracle in fp64 from the fp32-rounded inputs with its own dt sequence (R16)."""
+    f, meta = inputs.blast3d(128) if name == "c3" else inputs.turbulence(128, 128, 128)
+    gamma, bc = meta["gamma"], meta["bc"]
+    ref = _ref_input(f, "f32")
+    s = _solver(B, f, gamma, bc, "f32")
+    for k in range(100):
+        dt = 0.8 / oracle.cmax(ref, gamma, bc)
+        oracle.step_fixed(ref, gamma, bc, k, dt)
+        s.step_fixed(1, dt)
+    got = s.get_state()
+    s.close()
+    e = l1_rel(got, ref)
+    print(name, "128^3 fp32, L1 relative distance to the fp64 oracle after 100 steps:", e)
+    assert worst(e) <= TOL32_L1_100, e
+
+
 def test_conservation_and_divb_on_gpu_fp64(B):
     f, meta = inputs.turbulence(32, 32, 32)
     s = _solver(B, f, meta["gamma"], meta["bc"], "f64")

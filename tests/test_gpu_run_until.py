@@ -160,6 +160,30 @@ def test_graph_replay_is_bitwise_the_stream_path(B, shape, bc, prec):
         assert np.array_equal(x, y)
 
 
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_small_grid_bound_to_the_default_stream(B, prec):
+    """mhd_bind(workspace, NULL stream): the legacy default stream cannot be captured, so a small grid (where steps are
+    otherwise replayed as CUDA graphs) must launch its kernels directly; same bits as graph = 0 on an own stream"""
+    import torch
+    shape = (64, 16, 16)
+    f = [np.asarray(x, dtype=np.float32 if prec == "f32" else np.float64) for x in random_state(*shape, seed=5)]
+    ws = torch.empty(B.mhd_workspace_bytes(*shape, B.MHD_F32 if prec == "f32" else B.MHD_F64), dtype=torch.uint8, device="cuda")
+    a = B.Solver(*shape, 1.4, prec, P, workspace=ws)          # no stream: binds NULL
+    a.set_state(f)
+    ta = a.step(3, 0.8)
+    ra, sa = a.run_until(ta + 2.0, 0.8)
+    ga = a.get_state()
+    a.close()
+    b = _solver(B, f, 1.4, P, prec, graph=0)
+    tb = b.step(3, 0.8)
+    rb, sb = b.run_until(tb + 2.0, 0.8)
+    gb = b.get_state()
+    b.close()
+    assert ta == tb and ra == rb and sa == sb
+    for x, y in zip(ga, gb):
+        assert np.array_equal(x, y)
+
+
 @pytest.mark.parametrize("shape,prec", [((256, 64, 1), "f32"), ((256, 64, 1), "f64"), ((128, 16, 40), "f32"),
                                         ((128, 40, 16), "f64"), ((512, 1, 1), "f64")])
 @pytest.mark.parametrize("bc", [P, O])

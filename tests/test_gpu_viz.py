@@ -82,6 +82,12 @@ def test_viz_follows_the_state_and_edge_cases(env):
     s.viz_slice(1, 0, lo, hi, lut_d, img)
     torch.cuda.synchronize()
     assert tuple(img.cpu().numpy()[3, 5]) == tuple(lut[0])
+    # +-Inf cells are skipped by the range as well (mhd.h: smallest and largest FINITE value)
+    st[1][0, 7, 9] = np.inf
+    st[1][0, 8, 2] = -np.inf
+    s.set_state(st)
+    lo2, hi2 = s.viz_range(1)
+    assert (lo2, hi2) == (lo, hi) == viz.value_range(st, 1, meta["gamma"], meta["bc"])
     # argument errors
     for bad in (lambda: s.viz_slice(9, 0, 0.0, 1.0, lut_d, img), lambda: s.viz_slice(0, 1, 0.0, 1.0, lut_d, img),
                 lambda: s.viz_slice(0, 0, 1.0, 1.0, lut_d, img), lambda: s.viz_volume(0, 0.0, 1.0, lut_d, 0.0, img),
