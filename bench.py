@@ -280,11 +280,17 @@ def main():
         dtv, _ = sol.cfl_dt(CFL)
         kinds = [("fluid_x", B.MHD_OP_FLUID, 0, 13), ("fluid_y", B.MHD_OP_FLUID, 1, 13), ("fluid_z", B.MHD_OP_FLUID, 2, 13),
                  ("bpair_x", B.MHD_OP_BPAIR, 0, 8), ("bpair_y", B.MHD_OP_BPAIR, 1, 8), ("bpair_z", B.MHD_OP_BPAIR, 2, 8),
-                 ("lrev_x", B.MHD_OP_SWEEP_REVERSE, 0, 16)]   # reverse L_x: one fused kernel (fp32) or B pair + fluid
+                 ("lrev_x", B.MHD_OP_SWEEP_REVERSE, 0, 16),   # reverse L_x: one fused kernel (fp32) or B pair + fluid
+                 # reverse L_y / L_z: one kernel (B pair -> fluid through shared memory); middle pair of a step:
+                 # fluid kernel + one kernel for B pair, B pair, fluid (13 + 16 words)
+                 ("lrev_y", B.MHD_OP_SWEEP_REVERSE, 1, 16), ("lrev_z", B.MHD_OP_SWEEP_REVERSE, 2, 16),
+                 ("mid_y", B.MHD_OP_MIDDLE_PAIR, 1, 29), ("mid_z", B.MHD_OP_MIDDLE_PAIR, 2, 29)]
         breakdown = {}
         reps = 5
         with torch.cuda.stream(stream):
             for name, op, d, words in kinds:
+                sol.set_state(state)                           # repeated single operators are not a stable scheme: start each kind
+                dtv, _ = sol.cfl_dt(CFL)                       # from the workload's initial state, dt at its CFL limit
                 sol.apply(op, d, 0, dtv)                       # warm
                 a, b = ev(), ev()
                 torch.cuda.synchronize()
@@ -297,6 +303,7 @@ def main():
                 breakdown[name] = {"ms": kms, "algo_GBps": words * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": words}
             # the stand-alone c_max pass (first step / after mhd_apply only; steps fuse it into their last kernel):
             # cmax_reuse = 0 makes every mhd_cfl_dt run the reduction instead of returning the cached c_max
+            sol.set_state(state)
             sol.set_option("cmax_reuse", 0)
             sol.cfl_dt(CFL)
             a, b = ev(), ev()

@@ -48,7 +48,7 @@ enum mhd_status {
   MHD_ENONFINITE = -4, /* the c_max reduction saw NaN/Inf or c_max <= 0 (state is poisoned) */
   MHD_ENOSTATE = -5    /* stepping or reading before mhd_set_state */
 };
-enum mhd_operator { MHD_OP_FLUID = 0, MHD_OP_BPAIR = 1, MHD_OP_SWEEP_FORWARD = 2, MHD_OP_SWEEP_REVERSE = 3 };
+enum mhd_operator { MHD_OP_FLUID = 0, MHD_OP_BPAIR = 1, MHD_OP_SWEEP_FORWARD = 2, MHD_OP_SWEEP_REVERSE = 3, MHD_OP_MIDDLE_PAIR = 4 };
 
 /* Bytes of device memory a context of this shape needs (two copies of the 8 fields for out-of-place
  * operators plus a small scalar block).  Returns 0 on invalid arguments. */
@@ -109,7 +109,9 @@ int mhd_run_until(mhd_ctx* ctx, double t_end, double cfl, long long max_steps, l
 /* One operator of the step, for per-operator parity tests: op = MHD_OP_FLUID (fluid_d, Algorithm 1,
  * PAPER.md:273-285), MHD_OP_BPAIR (B_{t1->d} then B_{t2->d}, or t2 then t1 if reverse != 0;
  * Algorithm 2), MHD_OP_SWEEP_FORWARD / MHD_OP_SWEEP_REVERSE (L_d, PAPER.md:162,
- * 317; `reverse` is ignored).  d = 0, 1, 2 for x, y, z.  Does not synchronise. */
+ * 317; `reverse` is ignored), MHD_OP_MIDDLE_PAIR (forward L_d followed by reverse L_d, the third and fourth
+ * operator of every step, eqs (23)-(25) PAPER.md:164-170; `reverse` is ignored).  d = 0, 1, 2 for x, y, z.
+ * Does not synchronise. */
 int mhd_apply(mhd_ctx* ctx, int op, int d, int reverse, double dt);
 
 /* Step index s selects the sweep order (x,y,z), (z,x,y), (y,z,x) for s mod 3 = 0, 1, 2. */
@@ -161,6 +163,9 @@ int mhd_viz_volume(mhd_ctx* ctx, int field, double vmin, double vmax, const unsi
 /* Tuning knobs, all optional; none changes what is computed beyond rounding order inside the stated tolerances.
  *   "graph"   -1 auto (default: grids of <= 2^22 cells) | 0 | 1: replay whole steps of mhd_step / mhd_run_until
  *             as CUDA graphs (small grids are bound by launch latency)
+ *   "fuse"    sweeps along y, z on periodic grids: 1 (default) reverse L_d (B pair + fluid) and the middle pair of a step
+ *             (B pair + B pair + fluid) run as one kernel each | 2 the middle pair fuses its two B pairs only | 0 off
+ *   "cmax_reuse" 1 (default) mhd_cfl_dt returns the cached c_max while the state is unchanged | 0 always reduces
  *   "path"    0 auto (default) | 1 generic marching kernels only (any extents, both BCs)
  *   "segment" cells per block along the sweep for the marching kernels (-1 auto, 0 = whole pencil)
  *   "block"   threads per block of the generic kernels (multiple of 32 in [32, 256])

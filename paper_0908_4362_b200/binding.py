@@ -30,7 +30,7 @@ MHD_F32, MHD_F64 = 0, 1
 MHD_BC_PERIODIC, MHD_BC_OUTFLOW = 0, 1
 MHD_HOST, MHD_DEVICE = 0, 1
 MHD_OK, MHD_EINVAL, MHD_ENOMEM, MHD_ECUDA, MHD_ENONFINITE, MHD_ENOSTATE = 0, -1, -2, -3, -4, -5
-MHD_OP_FLUID, MHD_OP_BPAIR, MHD_OP_SWEEP_FORWARD, MHD_OP_SWEEP_REVERSE = 0, 1, 2, 3
+MHD_OP_FLUID, MHD_OP_BPAIR, MHD_OP_SWEEP_FORWARD, MHD_OP_SWEEP_REVERSE, MHD_OP_MIDDLE_PAIR = 0, 1, 2, 3, 4
 
 # every symbol include/mhd.h declares: (restype, argtypes)
 _P8 = POINTER(c_void_p)

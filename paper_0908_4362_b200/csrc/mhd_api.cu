@@ -18,6 +18,7 @@
 #include "mhd_yz2.cuh"
 #include "mhd_bring.cuh"
 #include "mhd_x2.cuh"
+#include "mhd_lrev.cuh"
 #include "mhd_viz.cuh"
 
 using namespace mhd;
@@ -62,6 +63,7 @@ struct mhd_ctx {
   long long launches;
   // options
   int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages, opt_pack, opt_bring, opt_xpack, opt_xfuse;
+  int opt_fuse;            // fused reverse L_y / L_z and fused middle pair (mhd_lrev.cuh): 0 off, 1 on, 2 middle pair fuses the two B pairs only
   int opt_cmax_reuse;      // 1: mhd_cfl_dt returns the cached c_max when the state has not changed; 0: always reduce
   int opt_graph;           // -1 auto (small grids), 0 never, 1 always: replay whole steps as CUDA graphs
   StepGraph graphs[64];    // one per (step index mod 3, reduction flags, clip)
@@ -143,6 +145,7 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_xfuse = 1;
   c->opt_graph = -1;
   c->opt_cmax_reuse = 1;
+  c->opt_fuse = 1;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -594,6 +597,65 @@ static int launch_bpair_x(mhd_ctx* c, int t2_first) {
   return MHD_OK;
 }
 
+// ---- fused reverse L_d and fused middle pair for d = y, z (mhd_lrev.cuh) ---------------------------------------------
+// np: number of B passes (1: reverse L_d; 2: forward B pair + reverse B pair), fl: followed by the fluid update
+static bool lrev_ok(const mhd_ctx* c, int d) {
+  const int tile = c->precision == MHD_F32 ? 128 : 64;
+  return c->opt_fuse && c->opt_path == 0 && d != 0 && c->bc == MHD_BC_PERIODIC && c->n[d] >= 32 && c->n[0] % tile == 0 &&
+         c->N < ((size_t)1 << 31);
+}
+
+template <class real>
+static int launch_lrev(mhd_ctx* c, int d, int np, bool fl, bool want_cmax) {
+  constexpr bool f32 = std::is_same<real, float>::value;
+  using T = typename std::conditional<f32, f2, real>::type;
+  constexpr int TXB = f32 ? 128 : 64;
+  const int t1 = (d + 1) % 3, t2 = (d + 2) % 3, o = 3 - d;
+  const int stride[3] = {1, c->n[0], c->n[0] * c->n[1]};
+  LRevArgs<real> A;
+  memset(&A, 0, sizeof(A));
+  const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
+  for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
+  A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
+  A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];
+  A.dt = &c->sc->dt;
+  A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
+  A.nx = c->n[0]; A.nd = c->n[d]; A.no = c->n[o];
+  A.sd = stride[d]; A.so = stride[o];
+  A.x_is_t1 = (d == 2) ? 1 : 0;
+  A.t2_first[0] = np == 2 ? 0 : 1;            // middle pair: the forward operator's B pair comes first
+  A.t2_first[1] = 1;
+  A.gamma = (real)c->gamma;
+  const int minb = (np == 2 && fl) ? 2 : 3;
+  const int halo = 8 * np + (fl ? 7 : 0);
+  A.seg = c->opt_segment;
+  if (A.seg < 0) A.seg = pick_segment(A.nd, ((long long)A.nx / TXB) * A.no, (long long)c->sm_count * minb, halo);
+  if (A.seg == 0 || A.seg > A.nd) A.seg = A.nd;
+  if (A.seg < 16) A.seg = A.nd < 16 ? A.nd : 16;
+  const dim3 grid(A.nx / TXB, A.no, (A.nd + A.seg - 1) / A.seg);
+  void (*k)(const LRevArgs<real>) = nullptr;
+  size_t smem = 0;
+  const bool xt1 = A.x_is_t1 != 0;
+#define MHD_LREV_PICK(NP_, FL_)                                                                                        \
+  do {                                                                                                                 \
+    smem = LRevLayout<real, TXB, NP_, FL_>::smem_bytes();                                                              \
+    k = want_cmax ? (xt1 ? lrev_ring_kernel<real, T, TXB, NP_, FL_, true, true> : lrev_ring_kernel<real, T, TXB, NP_, FL_, false, true>) \
+                  : (xt1 ? lrev_ring_kernel<real, T, TXB, NP_, FL_, true, false> : lrev_ring_kernel<real, T, TXB, NP_, FL_, false, false>); \
+  } while (0)
+  if (np == 1) MHD_LREV_PICK(1, true);
+  else if (fl) MHD_LREV_PICK(2, true);
+  else { smem = LRevLayout<real, TXB, 2, false>::smem_bytes(); k = lrev_ring_kernel<real, T, TXB, 2, false, false, false>; }
+#undef MHD_LREV_PICK
+  const int nthr = (np + (fl ? 1 : 0)) * (TXB / PackOf<T>::L);
+  CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k<<<grid, nthr, smem, c->stream>>>(A);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  if (fl) for (int k2 = 0; k2 < 5; ++k2) { void* t = c->cur[role[k2]]; c->cur[role[k2]] = c->alt[role[k2]]; c->alt[role[k2]] = t; }
+  return MHD_OK;
+}
+
 // want_cmax: this is the last operator of a step; fuse the c_max reduction of the NEXT step into it.
 // *fused reports whether the kernel that ran could do so.
 template <class real>
@@ -681,8 +743,31 @@ static int sweep(mhd_ctx* c, int d, bool reverse, bool want_cmax = false, bool* 
     if (fused) *fused = want_cmax;
     return BY_PRECISION(c, launch_x2<float>(c, 2, 1, want_cmax), launch_x2<double>(c, 2, 1, want_cmax));
   }
+  if (c->n[d] > 1 && lrev_ok(c, d)) {                            // reverse L_y / L_z: B pair + fluid in one pass (mhd_lrev.cuh)
+    if (fused) *fused = want_cmax;
+    return BY_PRECISION(c, launch_lrev<float>(c, d, 1, true, want_cmax), launch_lrev<double>(c, d, 1, true, want_cmax));
+  }
   if ((rc = BY_PRECISION(c, launch_bpair<float>(c, d, 1), launch_bpair<double>(c, d, 1)))) return rc;
   return BY_PRECISION(c, launch_fluid<float>(c, d, want_cmax, fused), launch_fluid<double>(c, d, want_cmax, fused));
+}
+
+// The middle pair of a step: forward L_d followed by reverse L_d (eqs (23)-(25) PAPER.md:164-170: every step's third and
+// fourth operator share a direction) = fluid_d, B pair, B pair (t2 first), fluid_d.  For d = y, z the last three run as ONE
+// kernel (fuse = 2: the two B pairs only).
+static int middle_pair(mhd_ctx* c, int d, bool want_cmax = false, bool* fused = nullptr) {
+  int rc;
+  if (c->n[d] > 1 && lrev_ok(c, d)) {
+    c->acc_valid = c->fin_valid = false;
+    if ((rc = BY_PRECISION(c, launch_fluid<float>(c, d), launch_fluid<double>(c, d)))) return rc;
+    if (c->opt_fuse == 2) {
+      if ((rc = BY_PRECISION(c, launch_lrev<float>(c, d, 2, false, false), launch_lrev<double>(c, d, 2, false, false)))) return rc;
+      return BY_PRECISION(c, launch_fluid<float>(c, d, want_cmax, fused), launch_fluid<double>(c, d, want_cmax, fused));
+    }
+    if (fused) *fused = want_cmax;
+    return BY_PRECISION(c, launch_lrev<float>(c, d, 2, true, want_cmax), launch_lrev<double>(c, d, 2, true, want_cmax));
+  }
+  if ((rc = sweep(c, d, false))) return rc;
+  return sweep(c, d, true, want_cmax, fused);
 }
 
 // one double sweep, eqs (23)-(25) PAPER.md:164-170
@@ -692,10 +777,11 @@ static int double_sweep(mhd_ctx* c) {
   int rc;
   bool fused = false;
   if ((rc = arm_accumulator(c))) return rc;
-  for (int i = 0; i < 3; ++i) if ((rc = sweep(c, o[i], false))) return rc;
+  for (int i = 0; i < 2; ++i) if ((rc = sweep(c, o[i], false))) return rc;
+  if ((rc = middle_pair(c, o[2]))) return rc;
   // the last operator of the step (fluid of the reverse L along o[0]) also reduces c_max of the new
   // state, so the next step needs no separate pass over the 8 fields
-  for (int i = 2; i >= 0; --i) if ((rc = sweep(c, o[i], true, i == 0, &fused))) return rc;
+  for (int i = 1; i >= 0; --i) if ((rc = sweep(c, o[i], true, i == 0, &fused))) return rc;
   c->acc_valid = fused;
   if (fused) c->acc_dirty = true;
   c->step_index++;
@@ -877,6 +963,7 @@ extern "C" int mhd_apply(mhd_ctx* c, int op, int d, int reverse, double dt) {
       return BY_PRECISION(c, launch_bpair<float>(c, d, reverse ? 1 : 0), launch_bpair<double>(c, d, reverse ? 1 : 0));
     case MHD_OP_SWEEP_FORWARD: return sweep(c, d, false);
     case MHD_OP_SWEEP_REVERSE: return sweep(c, d, true);
+    case MHD_OP_MIDDLE_PAIR: return middle_pair(c, d);
     default: return fail(c, MHD_EINVAL, "mhd_apply: unknown operator %d", op);
   }
 }
@@ -1039,6 +1126,7 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   if (!strcmp(key, "pack")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "pack must be 0, 1, 128 or 256"); c->opt_pack = (int)value; return MHD_OK; }
   if (!strcmp(key, "xpack")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 0..3"); c->opt_xpack = (int)value; return MHD_OK; }
   if (!strcmp(key, "xfuse")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xfuse must be 0, 1 (fp32 only), 2 (always) or 3 (fp32, packed)"); c->opt_xfuse = (int)value; return MHD_OK; }
+  if (!strcmp(key, "fuse")) { if (value < 0 || value > 2) return fail(c, MHD_EINVAL, "fuse must be 0, 1 or 2"); c->opt_fuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "cmax_reuse")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "cmax_reuse must be 0 or 1"); c->opt_cmax_reuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "graph")) { if (value < -1 || value > 1) return fail(c, MHD_EINVAL, "graph must be -1 (auto), 0 or 1"); c->opt_graph = (int)value; return MHD_OK; }
   if (!strcmp(key, "path")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "path must be 0 or 1"); c->opt_path = (int)value; return MHD_OK; }

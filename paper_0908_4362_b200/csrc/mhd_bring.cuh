@@ -85,14 +85,24 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
 
   // ---- producer duty: one elected lane of the warp on duty issues the NCOPY copies of a stage; every operand is
   // warp-uniform (block indices, kernel parameters, the march step), so they are straight-line UBLKCPs (mhd_async.cuh)
+#ifdef MHD_EXP_L2FEED
+  const int om_off = ((o - 1) & 7) * A.so, o_off = (o & 7) * A.so, op_off = ((o + 1) & 7) * A.so;
+#else
   const int om_off = map_index1(o - 1, A.no, A.bc) * A.so, o_off = o * A.so, op_off = map_index1(o + 1, A.no, A.bc) * A.so;
+#endif
   const int cl = (xl / CH) * CH + o_off, cr = (xr / CH) * CH + o_off;     // the 16-byte chunks holding columns x0-1, x0+TXB of row o
   auto produce = [&](int itp) {                           // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
     if (elect_one()) {
+#ifdef MHD_EXP_L2FEED
+      // experiment: every block reads the same few rows, so the inputs come out of L2 (results are wrong on purpose)
+      const int od = (map_index1(n0 - 4 + itp, A.nd, A.bc) & 15) * A.sd;
+      const int odl = (map_index1(n0 - 8 + itp, A.nd, A.bc) & 15) * A.sd;
+#else
       const int od = map_index1(n0 - 4 + itp, A.nd, A.bc) * A.sd;
       const int odl = map_index1(n0 - 8 + itp, A.nd, A.bc) * A.sd;        // B_d of the cell finished at this step
+#endif
       real* st = ring + s * RG::STAGE;
       uint64_t* bar = &full[s];
       constexpr uint32_t RB = TXB * sizeof(real);

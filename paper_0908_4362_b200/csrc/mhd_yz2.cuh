@@ -73,7 +73,11 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
 
   // ---- producer duty: one elected lane of the warp on duty issues the 10 copies of a stage; every operand is
   // warp-uniform (block indices, kernel parameters, the march step), so the copies are straight-line UBLKCPs ------
+#ifdef MHD_EXP_L2FEED
+  const int rowbase = x0 + (o & 7) * A.so;       // experiment: inputs out of L2 (results are wrong on purpose)
+#else
   const int rowbase = x0 + o * A.so;
+#endif
   const int op_off = (map_index1(o + 1, A.no, A.bc) - o) * A.so;
   const int xchunk = (map_index1(x0 + TXB, A.nx, A.bc) / RG::CH) * RG::CH + o * A.so;   // B_x at x0+TXB lives in this 16-byte chunk
   auto produce = [&](int itp) {                          // called by one whole, converged warp
@@ -81,18 +85,35 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
     if (elect_one()) {
       const int q = n0 - 3 + itp;
+#ifdef MHD_EXP_L2FEED
+      const int od = (map_index1(q, A.nd, A.bc) & 15) * A.sd;
+      const int od1 = (map_index1(q + 1, A.nd, A.bc) & 15) * A.sd;
+#else
       const int od = map_index1(q, A.nd, A.bc) * A.sd;
       const int od1 = map_index1(q + 1, A.nd, A.bc) * A.sd;
+#endif
       real* st = ring + s * RG::STAGE;
       constexpr uint32_t RB = TXB * sizeof(real);
       mbar_expect_tx(&full[s], RG::BYTES);
+#ifdef MHD_EXP_CHEAPPROD
+      {   // experiment: ten copies from one base pointer with constant strides (same bytes, wrong rows)
+        const real* b0 = A.u[0] + od + rowbase;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) bulk_g2s(st + k * RG::ROW, b0 + k * 1024, RB, &full[s]);
+        bulk_g2s(st + 9 * RG::ROW, b0 + 9 * 1024, 16, &full[s]);
+        (void)od1; (void)op_off; (void)xchunk;
+      }
+      if (false)
+#endif
 #pragma unroll
       for (int k = 0; k < 5; ++k) bulk_g2s(st + k * RG::ROW, A.u[k] + od + rowbase, RB, &full[s]);
+#ifndef MHD_EXP_CHEAPPROD
       bulk_g2s(st + 5 * RG::ROW, A.bd + od1 + rowbase, RB, &full[s]);
       bulk_g2s(st + 6 * RG::ROW, A.bo + od + rowbase, RB, &full[s]);
       bulk_g2s(st + 7 * RG::ROW, A.bo + od + rowbase + op_off, RB, &full[s]);
       bulk_g2s(st + 8 * RG::ROW, A.bx + od + rowbase, RB, &full[s]);
       bulk_g2s(st + 9 * RG::ROW, A.bx + od + xchunk, 16, &full[s]);
+#endif
     }
     __syncwarp();
   };
