@@ -163,20 +163,15 @@ int mhd_viz_volume(mhd_ctx* ctx, int field, double vmin, double vmax, const unsi
 /* Tuning knobs, all optional; none changes what is computed beyond rounding order inside the stated tolerances.
  *   "graph"   -1 auto (default: grids of <= 2^22 cells) | 0 | 1: replay whole steps of mhd_step / mhd_run_until
  *             as CUDA graphs (small grids are bound by launch latency)
- *   "fuse"    sweeps along y, z on periodic grids: 1 (default) reverse L_d (B pair + fluid) and the middle pair of a step
- *             (B pair + B pair + fluid) run as one kernel each | 2 the middle pair fuses its two B pairs only | 0 off
+ *   "fuse"    sweeps along y, z on periodic grids: 0 (default) two kernels per L_d | 1 reverse L_d (B pair + fluid) and the
+ *             middle pair of a step (B pair + B pair + fluid) run as one kernel each | 2 the middle pair fuses its two B
+ *             pairs only.  Measured slower than the two-kernel path on B200, hence not the default.
  *   "cmax_reuse" 1 (default) mhd_cfl_dt returns the cached c_max while the state is unchanged | 0 always reduces
  *   "path"    0 auto (default) | 1 generic marching kernels only (any extents, both BCs)
  *   "segment" cells per block along the sweep for the marching kernels (-1 auto, 0 = whole pencil)
  *   "block"   threads per block of the generic kernels (multiple of 32 in [32, 256])
- *   "pack"    fluid y/z ring kernel: 0 off | 1 auto (default; fp32: two pencils per thread in packed f32x2
- *             arithmetic) | 128 | 256 columns per block
- *   "bring"   B-pair y/z ring kernel: 0 off | 1 auto (default) | 128 | 256 columns per block
- *   "ftma"    stages of the older TMA-ring y/z fluid kernel (0 off, 4, 6, 8); used when "pack" = 0
- *   "btile"   tile shape of the tile-march y/z B-pair kernel (0 off, 1 = 32x8, 2 = 64x8, 3 = 64x4, 4 = 128x4);
- *             used when "bring" = 0
- *   "btma", "bstages"  TMA variant of the tile march (0 off) and its ring depth (4, 6, 8)
- *   "xpack"   x kernels: 0 scalar mhd_x.cuh | 1 all packed | 2 all one row per thread (default) | 3 packed fluid_x only
+ *   "xpack"   x kernels: 1 two rows per thread in packed f32x2 arithmetic (fp32, even ny) | 2 one row per thread (default)
+ *             | 3 packed fluid_x only
  *   "xfuse"   reverse L_x in one kernel: 0 off | 1 fp32 only (default) | 2 always | 3 fp32, packed
  * Unknown keys and out-of-range values return MHD_EINVAL. */
 int mhd_set_option(mhd_ctx* ctx, const char* key, long long value);

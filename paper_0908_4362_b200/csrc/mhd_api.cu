@@ -10,11 +10,6 @@
 #include <type_traits>
 
 #include "mhd_generic.cuh"
-#include "mhd_yz.cuh"
-#include "mhd_x.cuh"
-#include "mhd_btile.cuh"
-#include "mhd_yz_tma.cuh"
-#include "mhd_btma.cuh"
 #include "mhd_yz2.cuh"
 #include "mhd_bring.cuh"
 #include "mhd_x2.cuh"
@@ -62,7 +57,9 @@ struct mhd_ctx {
   long long step_index;
   long long launches;
   // options
-  int opt_segment, opt_block, opt_path, opt_btile, opt_ftma, opt_btma, opt_bstages, opt_pack, opt_bring, opt_xpack, opt_xfuse;
+  int opt_segment, opt_block, opt_path, opt_xpack, opt_xfuse;
+  const void* smem_set[48];   // kernels whose dynamic shared-memory limit has been raised on this context's device
+  int n_smem_set;
   int opt_fuse;            // fused reverse L_y / L_z and fused middle pair (mhd_lrev.cuh): 0 off, 1 on, 2 middle pair fuses the two B pairs only
   int opt_cmax_reuse;      // 1: mhd_cfl_dt returns the cached c_max when the state has not changed; 0: always reduce
   int opt_graph;           // -1 auto (small grids), 0 never, 1 always: replay whole steps as CUDA graphs
@@ -135,17 +132,11 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_segment = -1;   // auto
   c->opt_block = 128;
   c->opt_path = 0;
-  c->opt_btile = 1;
-  c->opt_ftma = 8;
-  c->opt_btma = 0;
-  c->opt_bstages = 6;
-  c->opt_pack = 1;
-  c->opt_bring = 1;
   c->opt_xpack = 2;
   c->opt_xfuse = 1;
   c->opt_graph = -1;
   c->opt_cmax_reuse = 1;
-  c->opt_fuse = 1;
+  c->opt_fuse = 0;
   c->sm_count = 148;
   *out = c;
   return MHD_OK;
@@ -281,11 +272,30 @@ static SweepGeom<real> make_geom(const mhd_ctx* c, int d) {
   return g;
 }
 
-// ---- fast path for sweeps along y and z (mhd_yz.cuh) ----------------------------------------
-static const int kYZBlock = 128;
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per kernel and context (the attribute is per device; a context
+// lives on one device), not on every launch
+static int want_smem(mhd_ctx* c, const void* kernel, size_t bytes) {
+  for (int i = 0; i < c->n_smem_set; ++i)
+    if (c->smem_set[i] == kernel) return MHD_OK;
+  CUDA_TRY(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  if (c->n_smem_set < (int)(sizeof(c->smem_set) / sizeof(c->smem_set[0]))) c->smem_set[c->n_smem_set++] = kernel;
+  return MHD_OK;
+}
+
+static void swap_fields(mhd_ctx* c, const int* f, int n) {
+  for (int i = 0; i < n; ++i) { void* t = c->cur[f[i]]; c->cur[f[i]] = c->alt[f[i]]; c->alt[f[i]] = t; }
+}
+static const int kBFields[3] = {5, 6, 7};
+
+// ---- ring marches for sweeps along y and z (mhd_yz2.cuh, mhd_bring.cuh) ------------------------
+// tile width in columns: fp32 256 (128 threads, two pencils each) when nx allows, else 128; fp64 128
+static int yz_tile(const mhd_ctx* c) {
+  if (c->precision == MHD_F32 && c->n[0] % 256 == 0) return 256;
+  return c->n[0] % 128 == 0 ? 128 : 0;
+}
 
 static bool yz_ok(const mhd_ctx* c, int d) {
-  return c->opt_path == 0 && d != 0 && c->n[d] >= 8 && c->n[0] >= 32 && c->N < ((size_t)1 << 31);
+  return c->opt_path == 0 && d != 0 && c->n[d] >= 8 && yz_tile(c) != 0 && c->N < ((size_t)1 << 31);
 }
 
 // Segment length along the sweep for a march kernel whose blocks cover `pencil_blocks` tiles of the transverse
@@ -304,7 +314,7 @@ static int pick_segment(int nd, long long pencil_blocks, long long slots, int ha
 }
 
 template <class real>
-static YZArgs<real> make_yz(mhd_ctx* c, int d, int tile_cells = 128, int blocks_per_sm = 4, int halo = 6) {
+static YZArgs<real> make_yz(mhd_ctx* c, int d, int tile, int blocks_per_sm, int halo) {
   const int o = 3 - d;                        // the other transverse axis (x is always one of them)
   const int stride[3] = {1, c->n[0], c->n[0] * c->n[1]};
   YZArgs<real> A;
@@ -316,204 +326,103 @@ static YZArgs<real> make_yz(mhd_ctx* c, int d, int tile_cells = 128, int blocks_
   A.gamma = (real)c->gamma;
   A.dt = &c->sc->dt;
   int seg = c->opt_segment;
-  if (seg < 0) {
-    const long long pencil_blocks = ((long long)A.nx * A.no + tile_cells - 1) / tile_cells;
-    seg = pick_segment(A.nd, pencil_blocks, (long long)c->sm_count * blocks_per_sm, halo);
-  }
+  if (seg < 0) seg = pick_segment(A.nd, ((long long)A.nx / tile) * A.no, (long long)c->sm_count * blocks_per_sm, halo);
   if (seg == 0 || seg > A.nd) seg = A.nd;
   A.seg = seg;
   return A;
 }
 
 template <class real>
-static dim3 yz_grid(const YZArgs<real>& A) {
-  return dim3((A.nx + kYZBlock - 1) / kYZBlock, A.no, (A.nd + A.seg - 1) / A.seg);
-}
-
-template <class real>
 static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
+  constexpr bool f32 = std::is_same<real, float>::value;
+  using T = typename std::conditional<f32, f2, real>::type;
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3, o = 3 - d;
-  YZArgs<real> A = make_yz<real>(c, d);
+  const int P = yz_tile(c);
+  YZArgs<real> A = make_yz<real>(c, d, P, MHD_YZ2_MINB * ((f32 && P == 128) ? 2 : 1), 6);
   const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
-  const int D = c->opt_ftma;
-  // ring march with u(q-1), u(q-3) re-read from the ring: fp32 two pencils per thread in packed f2
-  // arithmetic, fp64 one pencil per thread (mhd_yz2.cuh)
-  {
-    constexpr bool f32 = std::is_same<real, float>::value;
-    using T = typename std::conditional<f32, f2, real>::type;
-    int P = c->opt_pack == 1 ? (f32 && A.nx % 256 == 0 ? 256 : (A.nx % 128 == 0 ? 128 : 0))
-                             : (c->opt_pack > 1 && A.nx % c->opt_pack == 0 ? c->opt_pack : 0);
-    if (!f32 && P == 256) P = 128;
-    if (D && P) {
-      if (c->opt_segment < 0)
-        A.seg = pick_segment(A.nd, ((long long)A.nx / P) * A.no, (long long)c->sm_count * MHD_YZ2_MINB * ((f32 && P == 128) ? 2 : 1), 6);
-      const dim3 grid(A.nx / P, A.no, (A.nd + A.seg - 1) / A.seg);
-      void (*k)(const YZArgs<real>) = nullptr;
-      size_t smem = 0;
-      constexpr int DR = MHD_YZ2_STAGES;
-      if (P == 256) {
-        if constexpr (f32) {
-          smem = FluidRing<real, 256>::smem_bytes(DR);
-          k = want_cmax ? (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, true> : fluid_yz_ring_kernel<real, T, 256, DR, false, true>)
-                        : (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, false> : fluid_yz_ring_kernel<real, T, 256, DR, false, false>);
-        }
-      } else {
-        smem = FluidRing<real, 128>::smem_bytes(DR);
-        k = want_cmax ? (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, true> : fluid_yz_ring_kernel<real, T, 128, DR, false, true>)
-                      : (A.x_is_t1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, false> : fluid_yz_ring_kernel<real, T, 128, DR, false, false>);
-      }
-      CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k<<<grid, P / PackOf<T>::L, smem, c->stream>>>(A);
-      c->launches++;
-      CUDA_TRY(c, cudaGetLastError());
-      for (int k2 = 0; k2 < 5; ++k2) { void* t = c->cur[role[k2]]; c->cur[role[k2]] = c->alt[role[k2]]; c->alt[role[k2]] = t; }
-      return MHD_OK;
+  for (int k = 0; k < 5; ++k) A.src[k] = (const char*)A.u[k] - (const char*)A.u[0];
+  A.src[5] = (const char*)A.bd - (const char*)A.u[0];
+  A.src[6] = (const char*)A.bo - (const char*)A.u[0];
+  A.src[7] = (const char*)A.bx - (const char*)A.u[0];
+  const dim3 grid(A.nx / P, A.no, (A.nd + A.seg - 1) / A.seg);
+  void (*k)(const YZArgs<real>) = nullptr;
+  size_t smem = 0;
+  constexpr int DR = MHD_YZ2_STAGES;
+  const bool xt1 = A.x_is_t1 != 0;
+  if (P == 256) {
+    if constexpr (f32) {
+      smem = FluidRing<real, 256>::smem_bytes(DR);
+      k = want_cmax ? (xt1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, true> : fluid_yz_ring_kernel<real, T, 256, DR, false, true>)
+                    : (xt1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, false> : fluid_yz_ring_kernel<real, T, 256, DR, false, false>);
     }
+  } else {
+    smem = FluidRing<real, 128>::smem_bytes(DR);
+    k = want_cmax ? (xt1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, true> : fluid_yz_ring_kernel<real, T, 128, DR, false, true>)
+                  : (xt1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, false> : fluid_yz_ring_kernel<real, T, 128, DR, false, false>);
   }
-  // TMA bulk-copy ring (mhd_yz_tma.cuh) when rows are whole 16-byte aligned blocks, else register prefetch
-  const int TXB = A.nx % 128 == 0 ? 128 : (A.nx % 32 == 0 ? 32 : 0);
-  if (D && TXB && (A.nx * sizeof(real)) % 16 == 0) {
-    const dim3 grid(A.nx / TXB, A.no, (A.nd + A.seg - 1) / A.seg);
-    void (*k)(const YZArgs<real>) = nullptr;
-    size_t smem = 0;
-    if (TXB == 128) { smem = FluidRing<real, 128>::smem_bytes(D); k = D == 4 ? fluid_yz_tma_kernel<real, 128, 4> : (D == 8 ? fluid_yz_tma_kernel<real, 128, 8> : fluid_yz_tma_kernel<real, 128, 6>); }
-    else            { smem = FluidRing<real, 32>::smem_bytes(D);  k = D == 4 ? fluid_yz_tma_kernel<real, 32, 4>  : (D == 8 ? fluid_yz_tma_kernel<real, 32, 8>  : fluid_yz_tma_kernel<real, 32, 6>); }
-    CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k<<<grid, TXB + 32, smem, c->stream>>>(A);
-  } else
-  fluid_yz_kernel<real, kYZBlock><<<yz_grid(A), kYZBlock, 0, c->stream>>>(A);
+  int rc = want_smem(c, (const void*)k, smem);
+  if (rc) return rc;
+  k<<<grid, P / PackOf<T>::L, smem, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
-  for (int k = 0; k < 5; ++k) { void* t = c->cur[role[k]]; c->cur[role[k]] = c->alt[role[k]]; c->alt[role[k]] = t; }
+  swap_fields(c, role, 5);
   return MHD_OK;
 }
 
 template <class real>
 static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
+  constexpr bool f32 = std::is_same<real, float>::value;
+  using T = typename std::conditional<f32, f2, real>::type;
   const int o = 3 - d;
-  YZArgs<real> A = make_yz<real>(c, d, 256, 3, 8);
+  const int W = yz_tile(c);
+  YZArgs<real> A = make_yz<real>(c, d, W, MHD_BRING_MINB, 8);
   A.u[0] = (const real*)c->cur[0]; A.u[1] = (const real*)c->cur[1 + d];
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];
   A.t2_first = t2_first;
-  // barrier-free row march fed by a TMA ring, packed f2 arithmetic in fp32 (mhd_bring.cuh)
-  if (c->opt_bring) {
-    using T = typename std::conditional<std::is_same<real, float>::value, f2, real>::type;
-    const int W = c->opt_bring > 1 ? c->opt_bring : (std::is_same<real, float>::value && A.nx % 256 == 0 ? 256 : 128);
-    if (A.nx % W == 0 && (W == 128 || (W == 256 && std::is_same<real, float>::value))) {
-      if (c->opt_segment < 0)
-        A.seg = pick_segment(A.nd, ((long long)A.nx / W) * A.no, (long long)c->sm_count * MHD_BRING_MINB, 8);
-      const dim3 grid(A.nx / W, A.no, (A.nd + A.seg - 1) / A.seg);
-      constexpr int D = MHD_BRING_STAGES;
-      void (*k)(const YZArgs<real>) = nullptr;
-      size_t smem = 0;
-      int nthr = 0;
-      if (W == 256) {
-        if constexpr (std::is_same<real, float>::value) {
-          k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); nthr = 256 / PackOf<T>::L;
-        }
-      } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); nthr = 128 / PackOf<T>::L; }
-      CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k<<<grid, nthr, smem, c->stream>>>(A);
-      c->launches++;
-      CUDA_TRY(c, cudaGetLastError());
-      for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
-      return MHD_OK;
-    }
-  }
-  // TMA-fed tile march (mhd_btma.cuh) when rows are whole 16-byte aligned blocks and the extents tile evenly
-  {
-    static const int shp[5][2] = {{0, 0}, {32, 8}, {64, 4}, {128, 2}, {64, 8}};
-    const int TXs = shp[c->opt_btma][0], TOs = shp[c->opt_btma][1];
-    if (TXs && A.nx % TXs == 0 && A.no % TOs == 0 && (A.nx * sizeof(real)) % 16 == 0) {
-      const dim3 grid(A.nx / TXs, A.no / TOs, (A.nd + A.seg - 1) / A.seg);
-      const int D = c->opt_bstages;
-      void (*k)(const YZArgs<real>) = nullptr;
-      size_t smem = 0;
-      int nthr = 0;
-#define MHD_BTMA_CASE(ID, TX_, TO_)                                                                         \
-      case ID: smem = BRing<real, TX_, TO_>::smem_bytes(D); nthr = BRing<real, TX_, TO_>::NT + 32;            \
-        k = D == 4 ? bpair_tma_kernel<real, TX_, TO_, 4> : (D == 8 ? bpair_tma_kernel<real, TX_, TO_, 8> : bpair_tma_kernel<real, TX_, TO_, 6>); break;
-      switch (c->opt_btma) {
-        MHD_BTMA_CASE(1, 32, 8)
-        MHD_BTMA_CASE(2, 64, 4)
-        MHD_BTMA_CASE(3, 128, 2)
-        default: MHD_BTMA_CASE(4, 64, 8)
-      }
-#undef MHD_BTMA_CASE
-      CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k<<<grid, nthr, smem, c->stream>>>(A);
-      c->launches++;
-      CUDA_TRY(c, cudaGetLastError());
-      for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
-      return MHD_OK;
-    }
-  }
-  // tile march (mhd_btile.cuh) when the transverse extents tile evenly, else one thread per pencil
-  const int tshape[5][2] = {{0, 0}, {32, 8}, {64, 8}, {64, 4}, {128, 4}};
-  const int TXs = tshape[c->opt_btile][0], TOs = tshape[c->opt_btile][1];
-  if (TXs && A.nx % TXs == 0 && A.no % TOs == 0) {
-    const dim3 grid(A.nx / TXs, A.no / TOs, (A.nd + A.seg - 1) / A.seg);
-    switch (c->opt_btile) {
-      case 1: bpair_tile_kernel<real, 32, 8><<<grid, 9 * 32, 0, c->stream>>>(A); break;
-      case 2: bpair_tile_kernel<real, 64, 8><<<grid, 9 * 64, 0, c->stream>>>(A); break;
-      case 3: bpair_tile_kernel<real, 64, 4><<<grid, 5 * 64, 0, c->stream>>>(A); break;
-      default: bpair_tile_kernel<real, 128, 4><<<grid, 5 * 128, 0, c->stream>>>(A); break;
-    }
-  } else
-  bpair_yz_kernel<real, kYZBlock><<<yz_grid(A), kYZBlock, 0, c->stream>>>(A);
+  A.src[0] = 0;
+  A.src[1] = (const char*)A.u[1] - (const char*)A.u[0];
+  A.src[5] = (const char*)A.bd - (const char*)A.u[0];
+  A.src[6] = (const char*)A.bo - (const char*)A.u[0];
+  A.src[7] = (const char*)A.bx - (const char*)A.u[0];
+  const dim3 grid(A.nx / W, A.no, (A.nd + A.seg - 1) / A.seg);
+  constexpr int D = MHD_BRING_STAGES;
+  void (*k)(const YZArgs<real>) = nullptr;
+  size_t smem = 0;
+  if (W == 256) {
+    if constexpr (f32) { k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); }
+  } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); }
+  int rc = want_smem(c, (const void*)k, smem);
+  if (rc) return rc;
+  k<<<grid, W / PackOf<T>::L, smem, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
-  for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  swap_fields(c, kBFields, 3);
   return MHD_OK;
 }
 
-// ---- fast path for sweeps along x (mhd_x.cuh) -------------------------------------------------
-template <class real>
-static bool x_ok(const mhd_ctx* c) {
-  const int V = VecOf<real>::V;
-  return c->opt_path == 0 && c->bc == MHD_BC_PERIODIC && c->n[0] % V == 0 && c->n[0] / V <= 256 &&
-         c->N < ((size_t)1 << 31);
-}
-
-template <class real>
-static XArgs<real> make_x(mhd_ctx* c, int* block, unsigned* grid) {
-  const int V = VecOf<real>::V;
-  XArgs<real> A;
-  memset(&A, 0, sizeof(A));
-  A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2];
-  A.tpr = A.nx / V;
-  A.rpb = A.tpr >= 128 ? 1 : 128 / A.tpr;
-  const int nrows = A.ny * A.nz;
-  if (A.rpb > nrows) A.rpb = nrows;
-  A.gamma = (real)c->gamma;
-  A.dt = &c->sc->dt;
-  *block = A.tpr * A.rpb;
-  *grid = (unsigned)((nrows + A.rpb - 1) / A.rpb);
-  return A;
-}
-
-// ---- lane-pack x kernels and the fused reverse L_x (mhd_x2.cuh) ---------------------------------------
+// ---- sweeps along x and the fused reverse L_x (mhd_x2.cuh) ------------------------------------------------------
 // kind: 0 fluid_x, 1 B pair, 2 reverse L_x in one pass (B pair then fluid)
 template <class real>
 static bool x2_ok(const mhd_ctx* c, int kind) {
   constexpr bool f32 = std::is_same<real, float>::value;
-  if (!x_ok<real>(c) || c->n[0] / VecOf<real>::V > X2Block<real>::NT || c->n[2] > 65535) return false;
-  if (kind == 2) return c->opt_xfuse == 2 || ((c->opt_xfuse == 1 || c->opt_xfuse == 3) && f32);   // fp64: the fused kernel is slower than the pair (profiles/)
-  // xpack: 0 kernels of mhd_x.cuh; 1 packed f2 where possible (fp32, even ny), else mhd_x.cuh; 2 the scalar instantiation;
-  // 3 packed fluid_x (where possible), scalar B pair
-  if (c->opt_xpack >= 2) return true;
-  return f32 && c->opt_xpack == 1 && c->n[1] % 2 == 0;
+  const int V = VecOf<real>::V;
+  if (c->opt_path != 0 || c->bc != MHD_BC_PERIODIC || c->n[0] % V != 0 || c->n[0] / V > X2Block<real>::NT ||
+      c->n[2] > 65535 || c->N >= ((size_t)1 << 31))
+    return false;
+  // xfuse: 0 never | 1 fp32 only (default; in fp64 the fused kernel is slower than the pair) | 2 always | 3 fp32, packed
+  if (kind == 2) return c->opt_xfuse == 2 || ((c->opt_xfuse == 1 || c->opt_xfuse == 3) && f32);
+  return true;
 }
 
 template <class real>
 static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   constexpr bool f32 = std::is_same<real, float>::value;
   using T2 = typename std::conditional<f32, f2, real>::type;
-  // xfuse = 3: the fused operator in packed f2 arithmetic even when the single operators run scalar
+  // xpack: 1 two rows per thread in packed f2 arithmetic (fp32, even ny) | 2 one row per thread (default) | 3 packed fluid_x only
   // measured at 512^3 fp32: fluid_x one row per thread at six blocks per SM 1.21 ms, packed (two rows per thread,
   // three blocks per SM) 1.23; B pair one row per thread 0.89 ms, packed 1.14: the x kernels want occupancy
   const bool pack = f32 && c->n[1] % 2 == 0 && (c->opt_xpack == 1 || (c->opt_xpack == 3 && kind == 0) || (kind == 2 && c->opt_xfuse == 3));
@@ -546,54 +455,14 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
     k = kind == 0 ? fluid_x2_kernel<real, real> : (kind == 1 ? bpair_x2_kernel<real, real> : lrev_x2_kernel<real, real>);
   }
   const size_t smem = slots * NT * (pack ? 2 : 1) * sizeof(real);
-  CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(35 * NT * (f32 ? 2 : 1) * sizeof(real))));
+  int rc = want_smem(c, (const void*)k, 35 * NT * (f32 ? 2 : 1) * sizeof(real));
+  if (rc) return rc;
   k<<<grid, block, smem, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
-  if (kind != 1) for (int f = 0; f < 5; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
-  if (kind != 0) for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
-  return MHD_OK;
-}
-
-template <class real>
-static int launch_fluid_x(mhd_ctx* c, bool want_cmax) {
-  int block; unsigned grid;
-  XArgs<real> A = make_x<real>(c, &block, &grid);
-  const int role[5] = {0, 1, 2, 3, 4};
-  for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
-  A.bx = (const real*)c->cur[5]; A.by = (const real*)c->cur[6]; A.bz = (const real*)c->cur[7];
-  A.cmax_bits = want_cmax ? &c->sc->cmax_bits : nullptr;
-  const size_t smem = (size_t)35 * block * sizeof(real);
-  static bool attr_set = false;
-  if (!attr_set) {
-    CUDA_TRY(c, cudaFuncSetAttribute(fluid_x_kernel<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, 35 * 256 * (int)sizeof(real)));
-    attr_set = true;
-  }
-  fluid_x_kernel<real><<<grid, block, smem, c->stream>>>(A);
-  c->launches++;
-  CUDA_TRY(c, cudaGetLastError());
-  for (int k = 0; k < 5; ++k) { void* t = c->cur[role[k]]; c->cur[role[k]] = c->alt[role[k]]; c->alt[role[k]] = t; }
-  return MHD_OK;
-}
-
-template <class real>
-static int launch_bpair_x(mhd_ctx* c, int t2_first) {
-  int block; unsigned grid;
-  XArgs<real> A = make_x<real>(c, &block, &grid);
-  A.u[0] = (const real*)c->cur[0]; A.u[1] = (const real*)c->cur[1];
-  A.bx = (const real*)c->cur[5]; A.by = (const real*)c->cur[6]; A.bz = (const real*)c->cur[7];
-  A.bxo = (real*)c->alt[5]; A.byo = (real*)c->alt[6]; A.bzo = (real*)c->alt[7];
-  A.t2_first = t2_first;
-  const size_t smem = (size_t)24 * block * sizeof(real);
-  static bool attr_set = false;
-  if (!attr_set) {
-    CUDA_TRY(c, cudaFuncSetAttribute(bpair_x_kernel<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, 24 * 256 * (int)sizeof(real)));
-    attr_set = true;
-  }
-  bpair_x_kernel<real><<<grid, block, smem, c->stream>>>(A);
-  c->launches++;
-  CUDA_TRY(c, cudaGetLastError());
-  for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
+  static const int kUFields[5] = {0, 1, 2, 3, 4};
+  if (kind != 1) swap_fields(c, kUFields, 5);
+  if (kind != 0) swap_fields(c, kBFields, 3);
   return MHD_OK;
 }
 
@@ -647,12 +516,13 @@ static int launch_lrev(mhd_ctx* c, int d, int np, bool fl, bool want_cmax) {
   else { smem = LRevLayout<real, TXB, 2, false>::smem_bytes(); k = lrev_ring_kernel<real, T, TXB, 2, false, false, false>; }
 #undef MHD_LREV_PICK
   const int nthr = (np + (fl ? 1 : 0)) * (TXB / PackOf<T>::L);
-  CUDA_TRY(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int rc = want_smem(c, (const void*)k, smem);
+  if (rc) return rc;
   k<<<grid, nthr, smem, c->stream>>>(A);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
-  for (int f = 5; f < 8; ++f) { void* t = c->cur[f]; c->cur[f] = c->alt[f]; c->alt[f] = t; }
-  if (fl) for (int k2 = 0; k2 < 5; ++k2) { void* t = c->cur[role[k2]]; c->cur[role[k2]] = c->alt[role[k2]]; c->alt[role[k2]] = t; }
+  swap_fields(c, kBFields, 3);
+  if (fl) swap_fields(c, role, 5);
   return MHD_OK;
 }
 
@@ -665,7 +535,6 @@ static int launch_fluid(mhd_ctx* c, int d, bool want_cmax = false, bool* fused =
   if (c->n[d] == 1) return MHD_OK;   // both face fluxes of the only cell are identical: exact no-op (R10)
   if (yz_ok(c, d)) { if (fused) *fused = want_cmax; return launch_fluid_yz<real>(c, d, want_cmax); }
   if (d == 0 && x2_ok<real>(c, 0)) { if (fused) *fused = want_cmax; return launch_x2<real>(c, 0, 0, want_cmax); }
-  if (d == 0 && x_ok<real>(c)) { if (fused) *fused = want_cmax; return launch_fluid_x<real>(c, want_cmax); }
   FluidArgs<real> A;
   const int role[5] = {0, 1 + d, 1 + t1, 1 + t2, 4};
   for (int k = 0; k < 5; ++k) { A.u[k] = (const real*)c->cur[role[k]]; A.uo[k] = (real*)c->alt[role[k]]; }
@@ -687,7 +556,6 @@ static int launch_bpair(mhd_ctx* c, int d, int t2_first) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
   if (yz_ok(c, d)) return launch_bpair_yz<real>(c, d, t2_first);
   if (d == 0 && x2_ok<real>(c, 1)) return launch_x2<real>(c, 1, t2_first, false);
-  if (d == 0 && x_ok<real>(c)) return launch_bpair_x<real>(c, t2_first);
   BPairArgs<real> A;
   A.rho = (const real*)c->cur[0]; A.md = (const real*)c->cur[1 + d];
   A.bd = (const real*)c->cur[5 + d]; A.bt1 = (const real*)c->cur[5 + t1]; A.bt2 = (const real*)c->cur[5 + t2];
@@ -1118,13 +986,7 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
     if (value < 32 || value > 256 || (value & 31)) return fail(c, MHD_EINVAL, "block must be a multiple of 32 in [32,256]");
     c->opt_block = (int)value; return MHD_OK;
   }
-  if (!strcmp(key, "ftma")) { if (value != 0 && value != 4 && value != 6 && value != 8) return fail(c, MHD_EINVAL, "ftma must be 0, 4, 6 or 8"); c->opt_ftma = (int)value; return MHD_OK; }
-  if (!strcmp(key, "btma")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btma must be 0..4"); c->opt_btma = (int)value; return MHD_OK; }
-  if (!strcmp(key, "bstages")) { if (value != 4 && value != 6 && value != 8) return fail(c, MHD_EINVAL, "bstages must be 4, 6 or 8"); c->opt_bstages = (int)value; return MHD_OK; }
-  if (!strcmp(key, "btile")) { if (value < 0 || value > 4) return fail(c, MHD_EINVAL, "btile must be 0..4"); c->opt_btile = (int)value; return MHD_OK; }
-  if (!strcmp(key, "bring")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "bring must be 0, 1, 128 or 256"); c->opt_bring = (int)value; return MHD_OK; }
-  if (!strcmp(key, "pack")) { if (value != 0 && value != 1 && value != 128 && value != 256) return fail(c, MHD_EINVAL, "pack must be 0, 1, 128 or 256"); c->opt_pack = (int)value; return MHD_OK; }
-  if (!strcmp(key, "xpack")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 0..3"); c->opt_xpack = (int)value; return MHD_OK; }
+  if (!strcmp(key, "xpack")) { if (value < 1 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 1, 2 or 3"); c->opt_xpack = (int)value; return MHD_OK; }
   if (!strcmp(key, "xfuse")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xfuse must be 0, 1 (fp32 only), 2 (always) or 3 (fp32, packed)"); c->opt_xfuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "fuse")) { if (value < 0 || value > 2) return fail(c, MHD_EINVAL, "fuse must be 0, 1 or 2"); c->opt_fuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "cmax_reuse")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "cmax_reuse must be 0 or 1"); c->opt_cmax_reuse = (int)value; return MHD_OK; }

@@ -12,18 +12,18 @@
 //     pxA  B_x rows (faces) of its own L columns        pxE  B_x row of the column to its right (scalar)
 //     po   B_o row o                                     pop  B_o row o+1
 // The +1 rows (pxE, pop) supply the constraint update of B_d and are recomputed instead of
-// exchanged: compared with the tile march of mhd_btile.cuh that costs arithmetic (which packed f2
+// exchanged: compared with a tile march that exchanges fluxes behind a block barrier (round 1: 1.11 ms) that costs arithmetic (which packed f2
 // instructions make cheap) and buys a kernel with no __syncthreads, no shared-memory flux exchange, no
 // global LOAD address arithmetic in the consumers, and warps that drift freely up to the ring depth.
 // A stage is released as soon as its rows are in registers, so the producer runs D-1 march steps ahead
 // (ncu on a first version that re-read B_t(k-4) from the ring and so kept stages four steps longer showed
 // the consumers waiting on the full-barriers: 4 stages in flight do not cover the HBM latency).
 //
-// Requirements (else bpair_tile_kernel / bpair_yz_kernel run): nx % TXB == 0, extent along d >= 8.
+// Requirements (else bpair_march_kernel of mhd_generic.cuh runs): nx % TXB == 0, extent along d >= 8.
 #pragma once
 #include <type_traits>
+#include "mhd_args.cuh"
 #include "mhd_async.cuh"
-#include "mhd_btile.cuh"
 #include "mhd_pack_io.cuh"
 
 namespace mhd {
@@ -38,7 +38,7 @@ struct BRowRing {
   static size_t smem_bytes(int D) { return (size_t)D * STAGE * sizeof(real) + 2 * D * sizeof(uint64_t); }
 };
 
-// Measured at 512^3 fp32 (ms per launch; tile march of mhd_btile.cuh: 1.11): dedicated producer warp,
+// Measured at 512^3 fp32 (ms per launch; tile march with a block barrier: 1.11): dedicated producer warp,
 // 2 blocks/SM 1.17; rotating duty, 3 blocks/SM, 6-7 stages: no slack 1.05, slack 1-2 0.87; 2 blocks/SM,
 // 10 stages, slack 3 1.04; 4 blocks/SM (128 registers, spills) 1.55.
 #ifndef MHD_BRING_MINB
@@ -84,13 +84,16 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   __syncthreads();
 
   // ---- producer duty: one elected lane of the warp on duty issues the NCOPY copies of a stage; every operand is
-  // warp-uniform (block indices, kernel parameters, the march step), so they are straight-line UBLKCPs (mhd_async.cuh)
+  // warp-uniform (block indices, kernel parameters, the march step), so they are straight-line UBLKCPs (mhd_async.cuh).
+  // Sources are  rho + (march offset) + (row / chunk byte offset of this block) + A.src[field]  (A.src in the constant bank)
+  constexpr long long ES = (long long)sizeof(real);
 #ifdef MHD_EXP_L2FEED
-  const int om_off = ((o - 1) & 7) * A.so, o_off = (o & 7) * A.so, op_off = ((o + 1) & 7) * A.so;
+  const long long om_b = (long long)(((o - 1) & 7) * A.so + x0) * ES, o_b = (long long)((o & 7) * A.so + x0) * ES, op_b = (long long)(((o + 1) & 7) * A.so + x0) * ES;
 #else
-  const int om_off = map_index1(o - 1, A.no, A.bc) * A.so, o_off = o * A.so, op_off = map_index1(o + 1, A.no, A.bc) * A.so;
+  const long long om_b = (long long)(map_index1(o - 1, A.no, A.bc) * A.so + x0) * ES, o_b = (long long)(o * A.so + x0) * ES,
+                  op_b = (long long)(map_index1(o + 1, A.no, A.bc) * A.so + x0) * ES;
 #endif
-  const int cl = (xl / CH) * CH + o_off, cr = (xr / CH) * CH + o_off;     // the 16-byte chunks holding columns x0-1, x0+TXB of row o
+  const long long cl_b = o_b + (long long)((xl / CH) * CH - x0) * ES, cr_b = o_b + (long long)((xr / CH) * CH - x0) * ES;   // the 16-byte chunks holding columns x0-1, x0+TXB of row o
   auto produce = [&](int itp) {                           // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
@@ -106,24 +109,24 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
       real* st = ring + s * RG::STAGE;
       uint64_t* bar = &full[s];
       constexpr uint32_t RB = TXB * sizeof(real);
-      const real* rho = A.u[0] + od;
-      const real* md = A.u[1] + od;
+      const char* rho = reinterpret_cast<const char*>(A.u[0] + od);
+      const char* md = rho + A.src[1];
       mbar_expect_tx(bar, RG::BYTES);
-      bulk_g2s(st + 0 * P + CH, rho + om_off + x0, RB, bar);
-      bulk_g2s(st + 1 * P + CH, rho + o_off + x0, RB, bar);
-      bulk_g2s(st + 2 * P + CH, rho + op_off + x0, RB, bar);
-      bulk_g2s(st + 3 * P + CH, md + om_off + x0, RB, bar);
-      bulk_g2s(st + 4 * P + CH, md + o_off + x0, RB, bar);
-      bulk_g2s(st + 5 * P + CH, md + op_off + x0, RB, bar);
-      bulk_g2s(st + 6 * P + CH, A.bx + od + o_off + x0, RB, bar);
-      bulk_g2s(st + 7 * P + CH, A.bo + od + o_off + x0, RB, bar);
-      bulk_g2s(st + 8 * P + CH, A.bo + od + op_off + x0, RB, bar);
-      bulk_g2s(st + 9 * P + CH, A.bd + odl + o_off + x0, RB, bar);
-      bulk_g2s(st + 1 * P, rho + cl, 16, bar);
-      bulk_g2s(st + 1 * P + CH + TXB, rho + cr, 16, bar);
-      bulk_g2s(st + 4 * P, md + cl, 16, bar);
-      bulk_g2s(st + 4 * P + CH + TXB, md + cr, 16, bar);
-      bulk_g2s(st + 6 * P + CH + TXB, A.bx + od + cr, 16, bar);
+      bulk_g2s(st + 0 * P + CH, rho + om_b, RB, bar);
+      bulk_g2s(st + 1 * P + CH, rho + o_b, RB, bar);
+      bulk_g2s(st + 2 * P + CH, rho + op_b, RB, bar);
+      bulk_g2s(st + 3 * P + CH, md + om_b, RB, bar);
+      bulk_g2s(st + 4 * P + CH, md + o_b, RB, bar);
+      bulk_g2s(st + 5 * P + CH, md + op_b, RB, bar);
+      bulk_g2s(st + 6 * P + CH, rho + A.src[7] + o_b, RB, bar);
+      bulk_g2s(st + 7 * P + CH, rho + A.src[6] + o_b, RB, bar);
+      bulk_g2s(st + 8 * P + CH, rho + A.src[6] + op_b, RB, bar);
+      bulk_g2s(st + 9 * P + CH, reinterpret_cast<const char*>(A.u[0] + odl) + A.src[5] + o_b, RB, bar);
+      bulk_g2s(st + 1 * P, rho + cl_b, 16, bar);
+      bulk_g2s(st + 1 * P + CH + TXB, rho + cr_b, 16, bar);
+      bulk_g2s(st + 4 * P, md + cl_b, 16, bar);
+      bulk_g2s(st + 4 * P + CH + TXB, md + cr_b, 16, bar);
+      bulk_g2s(st + 6 * P + CH + TXB, rho + A.src[7] + cr_b, 16, bar);
     }
     __syncwarp();
   };

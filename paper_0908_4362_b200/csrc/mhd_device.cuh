@@ -313,4 +313,49 @@ struct BPipe {
   __device__ __forceinline__ real bold() const { return bold_; }
 };
 
+// Register pipeline of B_{t->d} for one row of faces (Algorithm 2; eqs (20)-(22)
+// PAPER.md:147-158) with all delay lines as circular arrays indexed by the march step modulo 4 (K is a
+// compile-time constant inside the 4x unrolled loop).  push<K>(vt(k), B_t(k)) finishes the second-order
+// edge flux f*dt at face (k-4)+1/2 and returns B_t'(k-4); flo is the flux at face (k-4)-1/2, fhi the new one.
+template <class real>
+struct BPipe4 {
+  real vt[2];        // vt(k-2), vt(k-1)            slot = step & 1
+  real b[4];         // B_t(k-4..k-1)               slot = step & 3
+  real w1[2];        // vg*B_t^{t+dt/2}(k-4), (k-3)  slot = step & 1
+  real vh[2];        // 2 * face velocity at (k-4)+1/2, (k-3)+1/2 (only the sign is used)
+  real vg, w0, f1, f;   // vg(k-2), vg*B_t(k-2), first-order flux at (k-3)+1/2, second-order flux*dt at (k-5)+1/2
+  real dw, sl;       // w1(k-3) - w1(k-4), and the limited slope of w1 at cell k-4 (see push)
+
+  __device__ __forceinline__ void init() {
+    vt[0] = vt[1] = vh[0] = vh[1] = vg = w0 = f1 = f = dw = sl = w1[0] = w1[1] = real(0);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = real(0);
+  }
+  __device__ __forceinline__ real fhi() const { return f; }     // after push: flux*dt at face (k-4)+1/2
+
+  template <int K>
+  __device__ __forceinline__ void push(real vtn, real btn, real dt, real hdt, real& bnew, real& flo) {
+    const real vg1 = real(0.25) * fma_(real(2), vt[(K + 1) & 1], vt[K & 1] + vtn);   // eq (20) at k-1
+    const real w01 = vg1 * b[(K + 3) & 3];
+    const real vh2 = vg + vg1;                                                       // 2 * eq (22) at face (k-2)+1/2
+    const real f1n = pick_pos(vh2, w0, w01);                                         // eq (21)
+    const real bh = fnma_(f1n - f1, hdt, b[(K + 2) & 3]);                            // Alg. 2 step 7: B_t^{t+dt/2}(k-2)
+    const real wD = vg * bh;
+    // Alg. 2 step 8: second-order TVD flux at face (k-4)+1/2 between the cells k-4 (wB) and k-3 (wC), upwinded by
+    // the sign of the face velocity there:  wB + vl(wB - wA, wC - wB)  or  wC + vl(wC - wD, wB - wC).
+    // vl(a, b) = ab / (a + b) is symmetric and odd under a common sign change, so the second form is wC - s(k-3)
+    // with s(c) = vl(w(c) - w(c-1), w(c+1) - w(c)), the limited slope AT a cell: s(k-3) is computed once here and
+    // serves the next face as s(k-4) (same products, same sums: the result has the same bits as selecting the three
+    // operands first, with one reciprocal per step as before and two selects fewer).
+    const real wB = w1[K & 1], wC = w1[(K + 1) & 1];
+    const real dn = wD - wC;
+    const real sn = vl_full(dw, dn);                                                 // s(k-3)
+    const real fn = pick_pos(vh[K & 1], wB + sl, wC - sn) * dt;
+    bnew = b[K & 3] - (fn - f);                                                      // Alg. 2 step 9 at cell k-4
+    flo = f;
+    f = fn; f1 = f1n; vg = vg1; w0 = w01; dw = dn; sl = sn;
+    vt[K & 1] = vtn; b[K & 3] = btn; w1[K & 1] = wD; vh[K & 1] = vh2;
+  }
+};
+
 }  // namespace mhd

@@ -215,7 +215,6 @@ lrev_ring_kernel(const LRevArgs<real> A) {
     int w4 = 0; uint32_t wph = 0;                                    // output ring (X1 for P1 when NP = 2, X2 for the last pass when FL)
     real* ringIn = first ? ringB : ringX1;
     uint64_t* fullIn = first ? fullB : fullX1;
-    uint64_t* emptyIn = first ? emptyB : emptyX1;
     constexpr int IN_STAGE = LY::B_STAGE;                            // = X_STAGE
     static_assert(LY::B_STAGE == LY::X_STAGE, "P1 and P2 share the input row layout");
     const bool to_ring = (NP == 2 && first) || (FL && last);
@@ -299,7 +298,7 @@ lrev_ring_kernel(const LRevArgs<real> A) {
       if (it >= 8) adv4(w4, wph, DOUT);
     }
     (void)bphprev;
-  } else if (FL) {
+  } else if constexpr (FL) {
     // =========================================== fluid update ========================================================
     const int rowbase = x0 + o * A.so;
     auto produceU = [&](int ord) {

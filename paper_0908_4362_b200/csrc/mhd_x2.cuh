@@ -1,12 +1,13 @@
 // mhd_x2.cuh -- sweeps along x (the contiguous axis), periodic boundaries, in lane-pack arithmetic, and the
 // fused reverse operator L_x^rev = B_{z->x}, B_{y->x}, fluid_x in ONE kernel.
 //
-// Same decomposition as mhd_x.cuh (a thread owns V consecutive cells of a row, a group of nx/V threads
-// covers the whole row so the periodic wrap is the group's own ring, neighbour values go through shared
-// memory, one barrier per stage, no halo cell recomputed), with two changes:
+// Along x the stencil runs along the lanes, so instead of marching a thread owns V consecutive cells of a row
+// (V = 4 floats or 2 doubles: every global access is one aligned 16-byte vector) and a group of nx/V threads
+// covers the whole row, so the periodic wrap is the group's own ring; the few stencil values a thread needs from
+// its neighbours go through shared memory, one barrier per stage, and no halo cell is recomputed.  Two refinements:
 //
 //  * T = f2 (mhd_pack.cuh): a thread owns the same V columns of TWO adjacent rows (j, j+1) and advances
-//    both with packed fp32 instructions (FADD2/FMUL2/FFMA2): the x kernels of mhd_x.cuh are issue-bound
+//    both with packed fp32 instructions (FADD2/FMUL2/FFMA2): the scalar x kernels are issue-bound
 //    (profiles/r01_c4_step_ncu_full_b.md: 273 and 194 issued instructions per cell, 65-68 % issue
 //    utilisation), and about 60 % of what they issue is FADD/FMUL/FFMA.  The shared-memory exchange moves
 //    8-byte packs (LDS.64/STS.64), so those instructions halve per cell as well.
@@ -19,11 +20,11 @@
 //    The FORWARD operator cannot be fused this way: its B pair needs the UPDATED rho, m_x of the four
 //    transverse neighbour rows, i.e. the fluid update of rows this block does not own.
 //
-// Requirements (else the kernels of mhd_x.cuh / mhd_generic.cuh run): periodic BC, nx % V == 0,
+// Requirements (else the generic kernels of mhd_generic.cuh run): periodic BC, nx % V == 0,
 // nx / V <= 256, N < 2^31, and for T = f2 an even ny.
 #pragma once
+#include "mhd_args.cuh"
 #include "mhd_pack_io.cuh"
-#include "mhd_x.cuh"
 
 namespace mhd {
 

@@ -129,8 +129,8 @@ def _gather3(fields, lo, dims):
     return out
 
 
-@pytest.mark.parametrize("nx,ny,nz,prec", [(1024, 256, 192, "f32"),     # widest row the x kernels take (falls back to
-                                                                       # mhd_x.cuh), four ring tiles per row
+@pytest.mark.parametrize("nx,ny,nz,prec", [(1024, 256, 192, "f32"),     # rows wider than the x kernels take (generic
+                                                                       # march along x), four ring tiles per row
                                            (384, 200, 136, "f32"),      # 128-wide ring tiles, extents that are no
                                            (384, 200, 136, "f64")])     # multiple of the segment or tile sizes
 def test_large_non_cubic_sampled_parity(nx, ny, nz, prec):

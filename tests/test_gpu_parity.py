@@ -359,65 +359,20 @@ def test_fused_cfl_reduction_paths(B):
     s.close()
 
 
-@pytest.mark.parametrize("btile", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("nx", [512, 384, 128])       # 256-wide ring tiles, 128-wide ring tiles, a single tile
 @pytest.mark.parametrize("bc", [P, O])
-@pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_b_pair_tile_shapes(B, btile, bc, prec):
-    """every tile shape of the y/z tile-march B kernel (and the per-pencil kernel, btile = 0), with segments"""
-    f0 = random_state(128, 16, 24, seed=77 + bc)
-    gamma, dt = 5.0 / 3.0, 0.19
-    tol = TOL64 if prec == "f64" else TOL32_STEP
-    for d in (1, 2):
-        for rev in (0, 1):
-            ref = _ref_input(f0, prec)
-            t1, t2 = (d + 1) % 3, (d + 2) % 3
-            for t in ((t2, t1) if rev else (t1, t2)):
-                oracle.badvect(ref, gamma, bc, d, t, dt)
-            for seg in (0, 9):
-                s = _solver(B, f0, gamma, bc, prec, btile=btile, btma=0, segment=seg)
-                s.apply(B.MHD_OP_BPAIR, d, rev, dt)
-                got = s.get_state()
-                s.close()
-                e = max_rel(got, ref)
-                assert worst(e) <= tol, (btile, bc, prec, d, rev, seg, e)
-
-
-@pytest.mark.parametrize("btma,stages", [(1, 4), (1, 6), (1, 8), (2, 6), (3, 6), (4, 6)])
-@pytest.mark.parametrize("bc", [P, O])
-@pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_b_pair_tma_tile_march(B, btma, stages, bc, prec):
-    """every tile shape / ring depth of the TMA-fed tile-march B kernel (mhd_btma.cuh), whole pencils and ragged segments"""
-    f0 = random_state(128, 16, 24, seed=91 + bc)
-    gamma, dt = 5.0 / 3.0, 0.19
-    tol = TOL64 if prec == "f64" else TOL32_STEP
-    for d in (1, 2):
-        for rev in (0, 1):
-            ref = _ref_input(f0, prec)
-            t1, t2 = (d + 1) % 3, (d + 2) % 3
-            for t in ((t2, t1) if rev else (t1, t2)):
-                oracle.badvect(ref, gamma, bc, d, t, dt)
-            for seg in (0, 9):
-                s = _solver(B, f0, gamma, bc, prec, btma=btma, bstages=stages, segment=seg)
-                s.apply(B.MHD_OP_BPAIR, d, rev, dt)
-                got = s.get_state()
-                s.close()
-                e = max_rel(got, ref)
-                assert worst(e) <= tol, (btma, stages, bc, prec, d, rev, seg, e)
-
-
-@pytest.mark.parametrize("pack", [0, 1, 128, 256])
-@pytest.mark.parametrize("bc", [P, O])
-def test_packed_fp32_kernels(B, pack, bc):
-    """fp32 kernels that advance two pencils per thread in packed f2 arithmetic (mhd_yz2.cuh, mhd_bring.cuh): every row width
-    they accept, several segments with a ragged tail, the fused c_max reduction, against the scalar path"""
-    nx, ny, nz = 512, 22, 19
+def test_packed_fp32_kernels(B, nx, bc):
+    """fp32 kernels that advance two pencils per thread in packed f2 arithmetic (mhd_yz2.cuh, mhd_bring.cuh): both tile
+    widths, several segments with a ragged tail, the fused c_max reduction"""
+    pack = nx
+    ny, nz = 22, 19
     f0 = random_state(nx, ny, nz, seed=77 + bc)
     gamma, dt = 5.0 / 3.0, 0.19
     for seg in (-1, 9):
         for s0 in range(3):
             ref = _ref_input(f0, "f32")
             oracle.step_fixed(ref, gamma, bc, s0, dt)
-            s = _solver(B, f0, gamma, bc, "f32", pack=pack, bring=pack, segment=seg)
+            s = _solver(B, f0, gamma, bc, "f32", segment=seg)
             s.step_index = s0
             s.step_fixed(1, dt)
             got = s.get_state()
@@ -429,7 +384,7 @@ def test_packed_fp32_kernels(B, pack, bc):
             assert abs(cmg - cm) <= 2e-6 * cm, (pack, bc, seg, s0, cmg, cm)
 
 
-@pytest.mark.parametrize("bring", [0, 1])
+@pytest.mark.parametrize("bring", [1])
 @pytest.mark.parametrize("bc", [P, O])
 def test_b_pair_ring_march_fp64(B, bring, bc):
     """the barrier-free B-pair row march (mhd_bring.cuh) in fp64, forward and reverse order, ragged segments"""
@@ -443,7 +398,7 @@ def test_b_pair_ring_march_fp64(B, bring, bc):
                 t1, t2 = (d + 1) % 3, (d + 2) % 3
                 for t in ((t2, t1) if rev else (t1, t2)):
                     oracle.badvect(ref, gamma, bc, d, t, dt)
-                s = _solver(B, f0, gamma, bc, "f64", bring=bring, segment=seg)
+                s = _solver(B, f0, gamma, bc, "f64", segment=seg)
                 s.apply(B.MHD_OP_BPAIR, d, rev, dt)
                 got = s.get_state()
                 s.close()
@@ -451,7 +406,7 @@ def test_b_pair_ring_march_fp64(B, bring, bc):
                 assert worst(e) <= TOL64, (bring, bc, seg, d, rev, e)
 
 
-@pytest.mark.parametrize("xpack,xfuse", [(0, 0), (1, 0), (0, 1), (1, 1), (2, 0), (2, 1), (3, 1), (3, 3), (2, 2)])
+@pytest.mark.parametrize("xpack,xfuse", [(1, 0), (1, 1), (2, 0), (2, 1), (3, 1), (3, 3), (2, 2)])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("shape", [(512, 6, 4), (64, 8, 6), (256, 7, 3), (32, 2, 1), (128, 4, 2)])
 def test_x_kernels_pack_and_fused_reverse(B, shape, prec, xpack, xfuse):
