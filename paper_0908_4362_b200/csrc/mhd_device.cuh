@@ -24,10 +24,12 @@ __device__ __forceinline__ int map_index(int q, int n, int bc) {
   }
   return q < 0 ? 0 : (q >= n ? n - 1 : q);
 }
-// same, valid only for -n <= q < 2n (one wrap), branch free
+// same, valid only for -n <= q < 2n (one wrap); both rules evaluated and one selected, so that the producers of the ring
+// kernels (uniform datapath, a dozen calls per stage) get straight-line code instead of a branch on bc with two arms
 __device__ __forceinline__ int map_index1(int q, int n, int bc) {
-  if (bc == BC_PERIODIC) return q < 0 ? q + n : (q >= n ? q - n : q);
-  return q < 0 ? 0 : (q >= n ? n - 1 : q);
+  const int per = q + ((q >> 31) & n) - (q >= n ? n : 0);
+  const int cl = min(max(q, 0), n - 1);
+  return bc == BC_PERIODIC ? per : cl;
 }
 
 // MHD_F32_IEEE (diagnostic builds only, R15): IEEE division and square root and no fused multiply-add in
@@ -107,6 +109,13 @@ __device__ __forceinline__ real vl_full(real a, real b) {
   const real ab = a * b;
   const real r = ab * rcp_(a + b);
   return pos_or_zero(ab, r);
+}
+// x + vl_full(a, b) with the correction folded into one multiply-add:  a b / (a + b) + x  where a*b > 0, else x
+template <class real>
+__device__ __forceinline__ real vl_add(real x, real a, real b) {
+  const real ab = a * b;
+  const real y = fma_(ab, rcp_(a + b), x);
+  return pick_pos(ab, y, x);
 }
 
 // Cell-centred field of one cell (held fixed through both stages) and what the two
@@ -248,9 +257,9 @@ struct FluidPipe {
       // step 8, eqs (11)-(15): right-going value at face (q-2)+1/2 from cells q-3,q-2,q-1;
       // left-going value at face (q-3)+1/2 from the same cells (mirror image)
       const real dRb = Rc[k] - Rb_[k];
-      const real Rp = Rb_[k] + vl_full(dRa_[k], dRb);
+      const real Rp = vl_add(Rb_[k], dRa_[k], dRb);
       const real dGb = Gb_[k] - Gc[k];
-      const real Gp = Gb_[k] + vl_full(dGb, dGa_[k]);
+      const real Gp = vl_add(Gb_[k], dGb, dGa_[k]);
       const real phi2 = Rp_[k] - Gp;                 // 2 * flux at face (q-3)+1/2
       out[k] = fnma_(phi2 - phi2_[k], hdt, um3[k]);  // step 9, eq (17) at cell q-3
       // shift the window by one cell
@@ -297,7 +306,7 @@ struct BPipe {
     const real wD = vg2_ * bh;
     // Alg. 2 step 8: second-order TVD flux at face (q-4)+1/2, upwinded by the sign of vhA_
     const real x = pick_pos(vhA_, wB_, wC_), y = pick_pos(vhA_, wA_, wD), z = pick_pos(vhA_, wC_, wB_);
-    const real f = x + vl_full(x - y, z - x);
+    const real f = vl_add(x, x - y, z - x);
     flo_ = f_;
     f_ = f * dt;
     bold_ = b4_;

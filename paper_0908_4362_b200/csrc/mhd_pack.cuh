@@ -48,6 +48,17 @@ __device__ __forceinline__ f2 sqrt_(f2 x) { return f2(sqrt_(x.v.x), sqrt_(x.v.y)
 __device__ __forceinline__ f2 abs_(f2 x) { return f2(fabsf(x.v.x), fabsf(x.v.y)); }
 __device__ __forceinline__ f2 pos_or_zero(f2 s, f2 r) { return f2(s.v.x > 0.0f ? r.v.x : 0.0f, s.v.y > 0.0f ? r.v.y : 0.0f); }
 __device__ __forceinline__ f2 pick_pos(f2 s, f2 a, f2 b) { return f2(s.v.x > 0.0f ? a.v.x : b.v.x, s.v.y > 0.0f ? a.v.y : b.v.y); }
+// x + a b / (a + b) where a*b > 0, else x (vl_add of mhd_device.cuh): products and sums packed, the reciprocal, the test and
+// the final multiply-add per lane, so that the select folds into a predicated FFMA (one instruction per lane instead of
+// half an FFMA2 plus an FSEL)
+__device__ __forceinline__ f2 vl_add(f2 x, f2 a, f2 b) {
+  const f2 ab = a * b, s = a + b;
+  const float rx = rcp_(s.v.x), ry = rcp_(s.v.y);
+  f2 y = x;
+  if (ab.v.x > 0.0f) y.v.x = fmaf(ab.v.x, rx, x.v.x);
+  if (ab.v.y > 0.0f) y.v.y = fmaf(ab.v.y, ry, x.v.y);
+  return y;
+}
 __device__ __forceinline__ f2 freeze_speed(f2 v, f2 t, f2 inv) {
   return f2(fabsf(v.v.x) + sqrt_(fabsf(t.v.x) * inv.v.x), fabsf(v.v.y) + sqrt_(fabsf(t.v.y) * inv.v.y));
 }

@@ -164,8 +164,8 @@ __device__ __forceinline__ void fluid_x_core(T* sm, int tid, int tl, int tr, con
     g[V + 1] = S(5, c, tr);
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-      const T Rp = r[v + 1] + vl_full(r[v + 1] - r[v], r[v + 2] - r[v + 1]);      // eqs (11)-(15)
-      const T Gp = g[v + 1] + vl_full(g[v + 1] - g[v + 2], g[v] - g[v + 1]);      // mirror image
+      const T Rp = vl_add(r[v + 1], r[v + 1] - r[v], r[v + 2] - r[v + 1]);        // eqs (11)-(15)
+      const T Gp = vl_add(g[v + 1], g[v + 1] - g[v + 2], g[v] - g[v + 1]);        // mirror image
       phi[v + 1][c] = Rp - Gp;
     }
     S(6, c, tid) = phi[V][c];        // my last face -> right neighbour's left face
@@ -252,7 +252,7 @@ __device__ __forceinline__ void bpair_x_core(T* sm, int tid, int tl, int tr, con
       const T x = pick_pos(vh[p][v], w1[p][v + 1], w1[p][v + 2]);
       const T y = pick_pos(vh[p][v], w1[p][v], w1[p][v + 3]);
       const T z = pick_pos(vh[p][v], w1[p][v + 2], w1[p][v + 1]);
-      f[p][v + 1] = (x + vl_full(x - y, z - x)) * dt;
+      f[p][v + 1] = vl_add(x, x - y, z - x) * dt;
     }
     S(1, p, tid) = f[p][V];
   }
