@@ -12,18 +12,39 @@ namespace mhd {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// MHD_JITTER (the second library build.py makes, libmhd_jitter.so; tests/test_gpu_jitter.py): every mbarrier wait, arrive and
+// expect_tx is preceded, about one time in sixteen, by a sleep of 0.2-2.2 us chosen from the clock and the warp's
+// position.  The march kernels have no block barrier; their warps drift and hand ring stages over through full/empty
+// mbarriers (the neighbour hazard of PAPER.md:319).  compute-sanitizer is closed on this pool, so the guard is this:
+// a protocol that only works for the interleavings the hardware happens to produce gives different bits (or hangs)
+// once the interleavings are scrambled, and the test demands identical bits.
+#ifdef MHD_JITTER
+__device__ __forceinline__ void jitter() {
+  unsigned t;
+  asm volatile("mov.u32 %0, %%clock;" : "=r"(t));
+  const unsigned w = (threadIdx.x >> 5) * 9u + blockIdx.x * 7u + blockIdx.y * 13u + blockIdx.z * 5u;
+  const unsigned h = (t * 2654435761u) ^ (w * 40503u);
+  if ((h >> 28) == 0u) __nanosleep(200u + ((h >> 8) & 2047u));
+}
+#else
+__device__ __forceinline__ void jitter() {}
+#endif
+
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
 __device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  jitter();
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  jitter();
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  jitter();
   asm volatile(
       "{\n"
       ".reg .pred p;\n"

@@ -101,7 +101,9 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   const long long xc_bytes = (long long)((map_index1(x0 + TXB, A.nx, A.bc) / RG::CH) * RG::CH - x0) * (long long)sizeof(real);   // B_x at x0+TXB lives in this 16-byte chunk
   auto produce = [&](int itp) {                          // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
+#ifndef MHD_BUG_NO_EMPTY_WAIT        // (fault injection for tests/test_gpu_jitter.py: refill a stage without waiting for its readers)
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
+#endif
     if (elect_one()) {
       const int q = n0 - 3 + itp;
 #ifdef MHD_EXP_L2FEED
