@@ -516,6 +516,24 @@ def test_cmax_negative_pressure_takes_the_absolute_value():
     assert abs(oracle.cmax(f, 2.0, P) - 2.0) < 1e-15
 
 
+def test_oracle_regression_fixture():
+    """tests/golden/oracle_tiny_state.txt (written by tests/golden/make_golden.py from the oracle alone) is reproduced
+    bit for bit: the oracle's arithmetic has not changed unnoticed"""
+    import os
+    from tests.golden import make_golden
+    want = {}
+    with open(os.path.join(os.path.dirname(make_golden.__file__), "oracle_tiny_state.txt")) as fh:
+        for line in fh:
+            if line.startswith("#"):
+                continue
+            tok = line.split()
+            want[(int(tok[0]), int(tok[1]))] = np.array([float.fromhex(t) for t in tok[2:]])
+    assert len(want) == 16
+    for bc in (0, 1):
+        for i, a in enumerate(make_golden.tiny_state(bc)):
+            assert np.array_equal(a.ravel(), want[(bc, i)]), (bc, i)
+
+
 def test_second_workload_set_generators():
     """initial data of the paper's E4 / E6: uniform B (div B = 0
     exactly), v = 0, p jump 10 / 0.1 at r = 0.1, and the oracle keeps the 2-D run 2-D"""
