@@ -170,6 +170,8 @@ int mhd_viz_volume(mhd_ctx* ctx, int field, double vmin, double vmax, const unsi
  *   "path"    0 auto (default) | 1 generic marching kernels only (any extents, both BCs)
  *   "segment" cells per block along the sweep for the marching kernels (-1 auto, 0 = whole pencil)
  *   "block"   threads per block of the generic kernels (multiple of 32 in [32, 256])
+ *   "brows"   B pair along y, z in fp32 on 256-column tiles: 2 (default) two rows per thread where the extent along the other
+ *             transverse axis is even | 1 one row per thread
  *   "xpack"   x kernels: 1 two rows per thread in packed f32x2 arithmetic (fp32, even ny) | 2 one row per thread (default)
  *             | 3 packed fluid_x only
  *   "xfuse"   reverse L_x in one kernel: 0 off | 1 fp32 only (default) | 2 always | 3 fp32, packed

@@ -57,7 +57,7 @@ struct mhd_ctx {
   long long step_index;
   long long launches;
   // options
-  int opt_segment, opt_block, opt_path, opt_xpack, opt_xfuse;
+  int opt_segment, opt_block, opt_path, opt_xpack, opt_xfuse, opt_brows;
   const void* smem_set[48];   // kernels whose dynamic shared-memory limit has been raised on this context's device
   int n_smem_set;
   int opt_fuse;            // fused reverse L_y / L_z and fused middle pair (mhd_lrev.cuh): 0 off, 1 on, 2 middle pair fuses the two B pairs only
@@ -134,6 +134,7 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_path = 0;
   c->opt_xpack = 2;
   c->opt_xfuse = 1;
+  c->opt_brows = 2;
   c->opt_graph = -1;
   c->opt_cmax_reuse = 1;
   c->opt_fuse = 0;
@@ -378,7 +379,15 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   using T = typename std::conditional<f32, f2, real>::type;
   const int o = 3 - d;
   const int W = yz_tile(c);
-  YZArgs<real> A = make_yz<real>(c, d, W, MHD_BRING_MINB, 8);
+  // brows = 2: two rows o, o+1 per thread (bpair_ring2_kernel): fp32, 256-column tiles, even extent along o
+  const bool two = f32 && c->opt_brows == 2 && W == 256 && c->n[o] % 2 == 0;
+  YZArgs<real> A = make_yz<real>(c, d, W, two ? 2 : MHD_BRING_MINB, 8);
+  if (two) {                                   // a block covers two rows: half as many pencil blocks
+    int seg = c->opt_segment;
+    if (seg < 0) seg = pick_segment(A.nd, ((long long)A.nx / W) * (A.no / 2), (long long)c->sm_count * 2, 8);
+    if (seg == 0 || seg > A.nd) seg = A.nd;
+    A.seg = seg;
+  }
   A.u[0] = (const real*)c->cur[0]; A.u[1] = (const real*)c->cur[1 + d];
   A.bd = (const real*)c->cur[5 + d]; A.bx = (const real*)c->cur[5]; A.bo = (const real*)c->cur[5 + o];
   A.bdo = (real*)c->alt[5 + d]; A.bxo = (real*)c->alt[5]; A.boo = (real*)c->alt[5 + o];
@@ -388,11 +397,13 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   A.src[5] = (const char*)A.bd - (const char*)A.u[0];
   A.src[6] = (const char*)A.bo - (const char*)A.u[0];
   A.src[7] = (const char*)A.bx - (const char*)A.u[0];
-  const dim3 grid(A.nx / W, A.no, (A.nd + A.seg - 1) / A.seg);
+  const dim3 grid(A.nx / W, two ? A.no / 2 : A.no, (A.nd + A.seg - 1) / A.seg);
   constexpr int D = MHD_BRING_STAGES;
   void (*k)(const YZArgs<real>) = nullptr;
   size_t smem = 0;
-  if (W == 256) {
+  if (two) {
+    if constexpr (f32) { k = bpair_ring2_kernel<256, MHD_BRING2_STAGES>; smem = BRowRing2<real, 256>::smem_bytes(MHD_BRING2_STAGES); }
+  } else if (W == 256) {
     if constexpr (f32) { k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); }
   } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); }
   int rc = want_smem(c, (const void*)k, smem);
@@ -987,6 +998,7 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
     c->opt_block = (int)value; return MHD_OK;
   }
   if (!strcmp(key, "xpack")) { if (value < 1 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 1, 2 or 3"); c->opt_xpack = (int)value; return MHD_OK; }
+  if (!strcmp(key, "brows")) { if (value < 1 || value > 2) return fail(c, MHD_EINVAL, "brows must be 1 or 2"); c->opt_brows = (int)value; return MHD_OK; }
   if (!strcmp(key, "xfuse")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xfuse must be 0, 1 (fp32 only), 2 (always) or 3 (fp32, packed)"); c->opt_xfuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "fuse")) { if (value < 0 || value > 2) return fail(c, MHD_EINVAL, "fuse must be 0, 1 or 2"); c->opt_fuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "cmax_reuse")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "cmax_reuse must be 0 or 1"); c->opt_cmax_reuse = (int)value; return MHD_OK; }

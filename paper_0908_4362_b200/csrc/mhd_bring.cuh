@@ -197,4 +197,179 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same march with TWO rows (o, o+1) per thread.  The flux row o+1 that the constraint step of row o needs (pop above)
+// is the thread's own row-o+1 pipeline, and the two scalar edge pipelines (pxE of either row) share ONE packed pipeline
+// whose lanes are the two rows: six packed pipelines for four pencils instead of eight, fifteen row copies per stage for two
+// rows instead of twenty, and every per-step cost (barrier waits, producer duty, loop, store offsets) once for two rows.
+// The price is registers: six pipelines are 192 registers of state, so two blocks of four warps per SM, each thread
+// with six independent dependency chains.  Requirements as above plus an even extent along o; fp32 (T = f2) only.
+//   stage rows: 0-3 rho(o-1..o+2)  4-7 m_d(o-1..o+2)  8,9 B_x(o, o+1)  10-12 B_o(o..o+2)  13,14 B_d(o, o+1) four cells behind
+//   chunks (columns x0-1 / x0+TXB): rho and m_d of rows o, o+1 (left and right), B_x of rows o, o+1 (right)
+// ---------------------------------------------------------------------------------------------------------------
+template <class real, int TXB>
+struct BRowRing2 {
+  static constexpr int CH = 16 / sizeof(real);
+  static constexpr int P = TXB + 2 * CH;
+  enum { ROWS = 15, NCHUNK = 10 };
+  static constexpr int STAGE = ROWS * P;
+  static constexpr uint32_t BYTES = ROWS * TXB * sizeof(real) + NCHUNK * 16;
+  static size_t smem_bytes(int D) { return (size_t)D * STAGE * sizeof(real) + 2 * D * sizeof(uint64_t); }
+};
+
+#ifndef MHD_BRING2_STAGES
+#define MHD_BRING2_STAGES 7
+#endif
+#ifndef MHD_BRING2_SLACK
+#define MHD_BRING2_SLACK 1
+#endif
+
+template <int TXB, int D>
+__global__ void __launch_bounds__(TXB / 2, 2) bpair_ring2_kernel(const YZArgs<float> A) {
+  typedef float real;
+  typedef f2 T;
+  typedef float S;
+  using RG = BRowRing2<real, TXB>;
+  constexpr int L = 2;
+  constexpr int NC = TXB / L;
+  constexpr int NW = NC / 32;
+  constexpr int PF = D - 1 - MHD_BRING2_SLACK;
+  constexpr int CH = RG::CH, P = RG::P;
+  static_assert(NW >= 1 && (NW & (NW - 1)) == 0 && NW <= 4, "block shape");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  real* ring = reinterpret_cast<real*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(ring + D * RG::STAGE);
+  uint64_t* empty = full + D;
+
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int x0 = blockIdx.x * TXB, o = 2 * blockIdx.y;
+  const int n0 = blockIdx.z * A.seg;
+  const int n1 = min(n0 + A.seg, A.nd);
+  const int niter = (n1 - n0 + 8 + 3) & ~3;
+  const int xl = map_index1(x0 - 1, A.nx, A.bc), xr = map_index1(x0 + TXB, A.nx, A.bc);
+  if (tid == 0) {
+    for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  constexpr long long ES = (long long)sizeof(real);
+  const long long om_b = (long long)(map_index1(o - 1, A.no, A.bc) * A.so + x0) * ES, o_b = (long long)(o * A.so + x0) * ES,
+                  o1_b = (long long)((o + 1) * A.so + x0) * ES, o2_b = (long long)(map_index1(o + 2, A.no, A.bc) * A.so + x0) * ES;
+  const long long cl_b = (long long)((xl / CH) * CH - x0) * ES, cr_b = (long long)((xr / CH) * CH - x0) * ES;   // chunk offsets inside a row
+  auto produce = [&](int itp) {
+    const unsigned s = (unsigned)itp % D;
+    if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
+    if (elect_one()) {
+      const int od = map_index1(n0 - 4 + itp, A.nd, A.bc) * A.sd;
+      const int odl = map_index1(n0 - 8 + itp, A.nd, A.bc) * A.sd;
+      real* st = ring + s * RG::STAGE;
+      uint64_t* bar = &full[s];
+      constexpr uint32_t RB = TXB * sizeof(real);
+      const char* rho = reinterpret_cast<const char*>(A.u[0] + od);
+      const char* md = rho + A.src[1];
+      const char* bx = rho + A.src[7];
+      const char* bo = rho + A.src[6];
+      const char* bd = reinterpret_cast<const char*>(A.u[0] + odl) + A.src[5];
+      mbar_expect_tx(bar, RG::BYTES);
+      bulk_g2s(st + 0 * P + CH, rho + om_b, RB, bar);
+      bulk_g2s(st + 1 * P + CH, rho + o_b, RB, bar);
+      bulk_g2s(st + 2 * P + CH, rho + o1_b, RB, bar);
+      bulk_g2s(st + 3 * P + CH, rho + o2_b, RB, bar);
+      bulk_g2s(st + 4 * P + CH, md + om_b, RB, bar);
+      bulk_g2s(st + 5 * P + CH, md + o_b, RB, bar);
+      bulk_g2s(st + 6 * P + CH, md + o1_b, RB, bar);
+      bulk_g2s(st + 7 * P + CH, md + o2_b, RB, bar);
+      bulk_g2s(st + 8 * P + CH, bx + o_b, RB, bar);
+      bulk_g2s(st + 9 * P + CH, bx + o1_b, RB, bar);
+      bulk_g2s(st + 10 * P + CH, bo + o_b, RB, bar);
+      bulk_g2s(st + 11 * P + CH, bo + o1_b, RB, bar);
+      bulk_g2s(st + 12 * P + CH, bo + o2_b, RB, bar);
+      bulk_g2s(st + 13 * P + CH, bd + o_b, RB, bar);
+      bulk_g2s(st + 14 * P + CH, bd + o1_b, RB, bar);
+      bulk_g2s(st + 1 * P, rho + o_b + cl_b, 16, bar);
+      bulk_g2s(st + 1 * P + CH + TXB, rho + o_b + cr_b, 16, bar);
+      bulk_g2s(st + 2 * P, rho + o1_b + cl_b, 16, bar);
+      bulk_g2s(st + 2 * P + CH + TXB, rho + o1_b + cr_b, 16, bar);
+      bulk_g2s(st + 5 * P, md + o_b + cl_b, 16, bar);
+      bulk_g2s(st + 5 * P + CH + TXB, md + o_b + cr_b, 16, bar);
+      bulk_g2s(st + 6 * P, md + o1_b + cl_b, 16, bar);
+      bulk_g2s(st + 6 * P + CH + TXB, md + o1_b + cr_b, 16, bar);
+      bulk_g2s(st + 8 * P + CH + TXB, bx + o_b + cr_b, 16, bar);
+      bulk_g2s(st + 9 * P + CH + TXB, bx + o1_b + cr_b, 16, bar);
+    }
+    __syncwarp();
+  };
+  for (int itp = warp; itp < PF && itp < niter; itp += NW) produce(itp);
+
+  const int cx = CH + L * tid;
+  const int iL = tid == 0 ? xl % CH : cx - 1;
+  const int iR = tid == NC - 1 ? CH + TXB + xr % CH : cx + L;
+  const S dts = (S)(*A.dt);
+  const T dt(dts), hdt(S(0.5) * dts);
+  const bool x_first = (A.x_is_t1 != 0) != (A.t2_first != 0);
+
+  BPipe4<T> pxA0, pxA1, pxE, po0, po1, po2;
+  pxA0.init(); pxA1.init(); pxE.init(); po0.init(); po1.init(); po2.init();
+  int off = (n0 - 8) * A.sd + x0 + L * tid + o * A.so;    // output cell m = q - 4 = n0 + it - 8, row o (row o+1: + A.so)
+  int stg = 0;
+  uint32_t ph = 0;
+
+  auto step = [&](auto Ktag, int it) {
+    constexpr int K = decltype(Ktag)::value;
+    if ((K & (NW - 1)) == warp && it + PF < niter) produce(it + PF);
+    const real* st = ring + stg * RG::STAGE;
+    mbar_wait(&full[stg], ph);
+    T* tag = nullptr;
+    const T r0 = ld_pack(st + 0 * P + cx, tag), r1 = ld_pack(st + 1 * P + cx, tag), r2 = ld_pack(st + 2 * P + cx, tag), r3 = ld_pack(st + 3 * P + cx, tag);
+    const T m0 = ld_pack(st + 4 * P + cx, tag), m1 = ld_pack(st + 5 * P + cx, tag), m2 = ld_pack(st + 6 * P + cx, tag), m3 = ld_pack(st + 7 * P + cx, tag);
+    const T rl(st[1 * P + iL], st[2 * P + iL]), rr(st[1 * P + iR], st[2 * P + iR]);      // lanes: rows o, o+1
+    const T ml(st[5 * P + iL], st[6 * P + iL]), mr(st[5 * P + iR], st[6 * P + iR]);
+    const T bx0 = ld_pack(st + 8 * P + cx, tag), bx1 = ld_pack(st + 9 * P + cx, tag);
+    const T bxr(st[8 * P + iR], st[9 * P + iR]);
+    const T bo0 = ld_pack(st + 10 * P + cx, tag), bo1 = ld_pack(st + 11 * P + cx, tag), bo2 = ld_pack(st + 12 * P + cx, tag);
+    const T bd0 = ld_pack(st + 13 * P + cx, tag), bd1 = ld_pack(st + 14 * P + cx, tag);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[stg]);
+    if (++stg == D) { stg = 0; ph ^= 1; }
+    // Alg. 2 step 4 (reading R5): face velocity = momentum sum / density sum of the two cells sharing the face
+    const T vtA0 = (shift_in_left(m1, ml.v.x) + m1) * rcp_(shift_in_left(r1, rl.v.x) + r1);
+    const T vtA1 = (shift_in_left(m2, ml.v.y) + m2) * rcp_(shift_in_left(r2, rl.v.y) + r2);
+    const T vtE = (T(m1.v.y, m2.v.y) + mr) * rcp_(T(r1.v.y, r2.v.y) + rr);       // the column right of my pack, rows o and o+1
+    const T vtO0 = (m0 + m1) * rcp_(r0 + r1);
+    const T vtO1 = (m1 + m2) * rcp_(r1 + r2);
+    const T vtO2 = (m2 + m3) * rcp_(r2 + r3);
+    T bxn0, bxn1, ben, bon0, bon1, bon2, fx0, fx1, fe, fo0, fo1, fo2;
+    pxA0.template push<K>(vtA0, bx0, dt, hdt, bxn0, fx0);
+    pxA1.template push<K>(vtA1, bx1, dt, hdt, bxn1, fx1);
+    pxE.template push<K>(vtE, bxr, dt, hdt, ben, fe);
+    po0.template push<K>(vtO0, bo0, dt, hdt, bon0, fo0);
+    po1.template push<K>(vtO1, bo1, dt, hdt, bon1, fo1);
+    po2.template push<K>(vtO2, bo2, dt, hdt, bon2, fo2);
+    const int m = n0 + it - 8;
+    if (it >= 8 && m < n1) {
+      st_pack(A.bxo + off, bxn0);                           // Alg. 2 step 9: advected B_t, rows o and o+1
+      st_pack(A.boo + off, bon0);
+      st_pack(A.bxo + off + A.so, bxn1);
+      st_pack(A.boo + off + A.so, bon1);
+      // constraint with the same fluxes at face m-1/2: columns x+1 and rows +1
+      const T cx0 = shift_in_right(fx0, fe.v.x) - fx0, cx1 = shift_in_right(fx1, fe.v.y) - fx1;
+      const T co0 = fo1 - fo0, co1 = fo2 - fo1;
+      T b0 = bd0, b1 = bd1;
+      if (x_first) { b0 = b0 + cx0; b0 = b0 + co0; b1 = b1 + cx1; b1 = b1 + co1; }
+      else         { b0 = b0 + co0; b0 = b0 + cx0; b1 = b1 + co1; b1 = b1 + cx1; }
+      st_pack(A.bdo + off, b0);
+      st_pack(A.bdo + off + A.so, b1);
+    }
+    off += A.sd;
+  };
+  for (int it = 0; it < niter; it += 4) {
+    step(std::integral_constant<int, 0>{}, it);
+    step(std::integral_constant<int, 1>{}, it + 1);
+    step(std::integral_constant<int, 2>{}, it + 2);
+    step(std::integral_constant<int, 3>{}, it + 3);
+  }
+}
+
 }  // namespace mhd

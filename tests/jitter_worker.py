@@ -13,7 +13,8 @@ import numpy as np
 # fused sweeps (fuse = 1, 2), short segments
 CASES = [((256, 24, 40), "f32", {}), ((256, 24, 40), "f64", {}), ((128, 40, 33), "f32", {"segment": 12}),
          ((128, 40, 36), "f32", {"fuse": 1}), ((128, 36, 40), "f64", {"fuse": 1}), ((256, 40, 36), "f32", {"fuse": 2}),
-         ((64, 40, 36), "f64", {"fuse": 1, "segment": 16}), ((512, 16, 12), "f32", {})]
+         ((64, 40, 36), "f64", {"fuse": 1, "segment": 16}), ((512, 16, 12), "f32", {}),
+         ((256, 24, 40), "f32", {"brows": 1})]          # the one-row fp32 B pair (default: two rows per thread)
 
 
 def run_all():

@@ -384,6 +384,34 @@ def test_packed_fp32_kernels(B, nx, bc):
             assert abs(cmg - cm) <= 2e-6 * cm, (pack, bc, seg, s0, cmg, cm)
 
 
+@pytest.mark.parametrize("shape", [(256, 14, 20), (512, 6, 10), (256, 2, 2), (768, 4, 12)])
+@pytest.mark.parametrize("bc", [P, O])
+def test_b_pair_two_rows_per_thread(B, shape, bc):
+    """bpair_ring2_kernel (mhd_bring.cuh; option brows = 2): two rows o, o+1 per thread, six packed flux pipelines for four
+    pencils.  Element-wise against the oracle, forward and reverse order, both directions, ragged segments; and against
+    the one-row kernel to a few ulp (the same arithmetic per cell; nvcc contracts a*b + c kernel by kernel)."""
+    nx, ny, nz = shape
+    f0 = random_state(nx, ny, nz, seed=123 + bc + nx)
+    gamma, dt = 5.0 / 3.0, 0.21
+    for seg in (-1, 9):
+        for d in (1, 2):
+            for rev in (0, 1):
+                ref = _ref_input(f0, "f32")
+                t1, t2 = (d + 1) % 3, (d + 2) % 3
+                for t in ((t2, t1) if rev else (t1, t2)):
+                    oracle.badvect(ref, gamma, bc, d, t, dt)
+                out = []
+                for brows in (2, 1):
+                    s = _solver(B, f0, gamma, bc, "f32", segment=seg, brows=brows)
+                    s.apply(B.MHD_OP_BPAIR, d, rev, dt)
+                    out.append(s.get_state())
+                    s.close()
+                e = max_rel(out[0], ref)
+                assert worst(e) <= TOL32_STEP, (shape, bc, seg, d, rev, e)
+                for a, b in zip(out[0], out[1]):
+                    assert np.max(np.abs(a - b)) <= 1e-6 * np.max(np.abs(b)), (shape, bc, seg, d, rev)
+
+
 @pytest.mark.parametrize("bring", [1])
 @pytest.mark.parametrize("bc", [P, O])
 def test_b_pair_ring_march_fp64(B, bring, bc):
