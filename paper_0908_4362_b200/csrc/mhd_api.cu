@@ -379,12 +379,12 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   using T = typename std::conditional<f32, f2, real>::type;
   const int o = 3 - d;
   const int W = yz_tile(c);
-  // brows = 2: two rows o, o+1 per thread (bpair_ring2_kernel): fp32, 256-column tiles, even extent along o
-  const bool two = f32 && c->opt_brows == 2 && W == 256 && c->n[o] % 2 == 0;
+  // brows = 2: two rows o, o+1 per thread (bpair_ring2_kernel): fp32, even extent along o
+  const bool two = f32 && c->opt_brows == 2 && c->n[o] % 2 == 0;
   YZArgs<real> A = make_yz<real>(c, d, W, two ? 2 : MHD_BRING_MINB, 8);
   if (two) {                                   // a block covers two rows: half as many pencil blocks
     int seg = c->opt_segment;
-    if (seg < 0) seg = pick_segment(A.nd, ((long long)A.nx / W) * (A.no / 2), (long long)c->sm_count * 2, 8);
+    if (seg < 0) seg = pick_segment(A.nd, ((long long)A.nx / W) * (A.no / 2), (long long)c->sm_count * (W == 256 ? 2 : 4), 8);
     if (seg == 0 || seg > A.nd) seg = A.nd;
     A.seg = seg;
   }
@@ -402,7 +402,10 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   void (*k)(const YZArgs<real>) = nullptr;
   size_t smem = 0;
   if (two) {
-    if constexpr (f32) { k = bpair_ring2_kernel<256, MHD_BRING2_STAGES>; smem = BRowRing2<real, 256>::smem_bytes(MHD_BRING2_STAGES); }
+    if constexpr (f32) {
+      if (W == 256) { k = bpair_ring2_kernel<256, MHD_BRING2_STAGES>; smem = BRowRing2<real, 256>::smem_bytes(MHD_BRING2_STAGES); }
+      else          { k = bpair_ring2_kernel<128, MHD_BRING2_STAGES>; smem = BRowRing2<real, 128>::smem_bytes(MHD_BRING2_STAGES); }
+    }
   } else if (W == 256) {
     if constexpr (f32) { k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); }
   } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); }

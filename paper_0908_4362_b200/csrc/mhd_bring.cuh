@@ -225,7 +225,7 @@ struct BRowRing2 {
 #endif
 
 template <int TXB, int D>
-__global__ void __launch_bounds__(TXB / 2, 2) bpair_ring2_kernel(const YZArgs<float> A) {
+__global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kernel(const YZArgs<float> A) {
   typedef float real;
   typedef f2 T;
   typedef float S;

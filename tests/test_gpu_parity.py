@@ -384,7 +384,7 @@ def test_packed_fp32_kernels(B, nx, bc):
             assert abs(cmg - cm) <= 2e-6 * cm, (pack, bc, seg, s0, cmg, cm)
 
 
-@pytest.mark.parametrize("shape", [(256, 14, 20), (512, 6, 10), (256, 2, 2), (768, 4, 12)])
+@pytest.mark.parametrize("shape", [(256, 14, 20), (512, 6, 10), (256, 2, 2), (768, 4, 12), (128, 10, 12), (384, 8, 6)])
 @pytest.mark.parametrize("bc", [P, O])
 def test_b_pair_two_rows_per_thread(B, shape, bc):
     """bpair_ring2_kernel (mhd_bring.cuh; option brows = 2): two rows o, o+1 per thread, six packed flux pipelines for four
