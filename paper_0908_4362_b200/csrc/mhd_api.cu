@@ -424,7 +424,7 @@ template <class real>
 static bool x2_ok(const mhd_ctx* c, int kind) {
   constexpr bool f32 = std::is_same<real, float>::value;
   const int V = VecOf<real>::V;
-  if (c->opt_path != 0 || c->bc != MHD_BC_PERIODIC || c->n[0] % V != 0 || c->n[0] / V > X2Block<real>::NT ||
+  if (c->opt_path != 0 || c->bc != MHD_BC_PERIODIC || c->n[0] % V != 0 || c->n[0] / V > X2Block<real>::NT_MAX ||
       c->n[2] > 65535 || c->N >= ((size_t)1 << 31))
     return false;
   // xfuse: 0 never | 1 fp32 only (default; in fp64 the fused kernel is slower than the pair) | 2 always | 3 fp32, packed
@@ -439,15 +439,17 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   // xpack: 1 two rows per thread in packed f2 arithmetic (fp32, even ny) | 2 one row per thread (default) | 3 packed fluid_x only
   // measured at 512^3 fp32: fluid_x one row per thread at six blocks per SM 1.21 ms, packed (two rows per thread,
   // three blocks per SM) 1.23; B pair one row per thread 0.89 ms, packed 1.14: the x kernels want occupancy
-  const bool pack = f32 && c->n[1] % 2 == 0 && (c->opt_xpack == 1 || (c->opt_xpack == 3 && kind == 0) || (kind == 2 && c->opt_xfuse == 3));
+  const bool pack = f32 && c->n[1] % 2 == 0 && c->n[0] / VecOf<real>::V <= X2Block<real>::NT && (c->opt_xpack == 1 || (c->opt_xpack == 3 && kind == 0) || (kind == 2 && c->opt_xfuse == 3));
   const int V = VecOf<real>::V, L = pack ? 2 : 1;
   XArgs<real> A;
   memset(&A, 0, sizeof(A));
   A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2];
   A.tpr = A.nx / V;
   A.tpr_shift = -1;
-  for (int b = 0; b < 9; ++b) if ((1 << b) == A.tpr) A.tpr_shift = b;
-  constexpr int NT = X2Block<real>::NT;
+  for (int b = 0; b < 11; ++b) if ((1 << b) == A.tpr) A.tpr_shift = b;
+  // block size: the smallest of NT, 2 NT, 4 NT threads that holds a whole row (packed variants: NT only)
+  constexpr int NT0 = X2Block<real>::NT;
+  const int NT = A.tpr <= NT0 ? NT0 : (A.tpr <= 2 * NT0 ? 2 * NT0 : 4 * NT0);
   A.one = (real)1;
   A.rpb = NT / A.tpr;
   const int gpp = A.ny / L;                          // row groups per plane
@@ -465,11 +467,17 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   const size_t slots = kind == 1 ? 24 : 35;
   if (pack) {
     if constexpr (f32) k = kind == 0 ? fluid_x2_kernel<real, T2> : (kind == 1 ? bpair_x2_kernel<real, T2> : lrev_x2_kernel<real, T2>);
-  } else {
+  } else if (NT == NT0) {
     k = kind == 0 ? fluid_x2_kernel<real, real> : (kind == 1 ? bpair_x2_kernel<real, real> : lrev_x2_kernel<real, real>);
+  } else if (NT == 2 * NT0) {
+    k = kind == 0 ? fluid_x2_kernel<real, real, 2 * NT0> : (kind == 1 ? bpair_x2_kernel<real, real, 2 * NT0> : lrev_x2_kernel<real, real, 2 * NT0>);
+  } else {
+    if constexpr (4 * NT0 <= X2Block<real>::NT_MAX)
+      k = kind == 0 ? fluid_x2_kernel<real, real, 4 * NT0> : (kind == 1 ? bpair_x2_kernel<real, real, 4 * NT0> : lrev_x2_kernel<real, real, 4 * NT0>);
   }
+  if (!k) return fail(c, MHD_EINVAL, "launch_x2: no kernel for %d threads per row", A.tpr);
   const size_t smem = slots * NT * (pack ? 2 : 1) * sizeof(real);
-  int rc = want_smem(c, (const void*)k, 35 * NT * (f32 ? 2 : 1) * sizeof(real));
+  int rc = want_smem(c, (const void*)k, 35 * (size_t)NT * (pack ? 2 : 1) * sizeof(real));
   if (rc) return rc;
   k<<<grid, block, smem, c->stream>>>(A);
   c->launches++;
@@ -577,6 +585,15 @@ static int launch_bpair(mhd_ctx* c, int d, int t2_first) {
   A.dt = &c->sc->dt;
   A.t2_first = t2_first;
   A.g = make_geom<real>(c, d);
+  if (c->n[d] == 1 && c->opt_path == 0) {      // extent 1 along the sweep: only the constraint term acts (bpair_flat_kernel)
+    A.g.seg = 1; A.g.nseg = 1;
+    const long long cells = (long long)A.g.na * A.g.nb;
+    bpair_flat_kernel<real><<<(unsigned)((cells + 255) / 256), 256, 0, c->stream>>>(A);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    void* t = c->cur[5 + d]; c->cur[5 + d] = c->alt[5 + d]; c->alt[5 + d] = t;
+    return MHD_OK;
+  }
   const long long threads = (long long)A.g.na * A.g.nb * A.g.nseg;
   const int block = c->opt_block;
   const unsigned grid = (unsigned)((threads + block - 1) / block);

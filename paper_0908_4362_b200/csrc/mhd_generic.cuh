@@ -138,6 +138,37 @@ __global__ void __launch_bounds__(256) bpair_march_kernel(const BPairArgs<real> 
   }
 }
 
+// B_{t1->d}, B_{t2->d} along an axis of extent 1 (the z sweeps of a 2-D problem, the y and z sweeps of a 1-D one).
+// Every index along d maps to the only cell under both boundary rules (reading R10), so in Algorithm 2
+// the smoothed velocity is vg = (vt + vt + 2 vt) / 4 = vt (exact), both first-order fluxes of a row are the same vg B_t,
+// the half step leaves B_t as it is, the limited differences vanish (a b = 0 is not > 0), and the edge flux is
+// f = (vg B_t) dt on both faces: B_t - (f - f) = B_t exactly, and only the constraint term f(tau+1) - f(tau) changes B_d
+// -- the d-derivative-free part of the induction equation that a 2-D run still needs.  One thread per
+// cell, no march, no warm-up; writes B_d only (the caller swaps that one field).
+template <class real>
+__global__ void __launch_bounds__(256) bpair_flat_kernel(const BPairArgs<real> A) {
+  const SweepGeom<real>& g = A.g;
+  int a, b, s;
+  if (!thread_to_pencil(g, a, b, s)) return;
+  const real dt = (real)(*A.dt);
+  const int am = map_index(a - 1, g.na, g.bc), ap = map_index(a + 1, g.na, g.bc);
+  const int bm = map_index(b - 1, g.nb, g.bc), bp = map_index(b + 1, g.nb, g.bc);
+  const long long o00 = a * g.sa + b * g.sb;
+  const long long om0 = am * g.sa + b * g.sb, op0 = ap * g.sa + b * g.sb;
+  const long long o0m = a * g.sa + bm * g.sb, o0p = a * g.sa + bp * g.sb;
+  const real r00 = A.rho[o00], m00 = A.md[o00];
+  // Alg. 2 step 4 (reading R5) for the rows tau and tau+1 of either transverse component, as in bpair_march_kernel
+  const real f1 = (((A.md[om0] + m00) * rcp_(A.rho[om0] + r00)) * A.bt1[o00]) * dt;
+  const real f1p = (((m00 + A.md[op0]) * rcp_(r00 + A.rho[op0])) * A.bt1[op0]) * dt;
+  const real f2 = (((A.md[o0m] + m00) * rcp_(A.rho[o0m] + r00)) * A.bt2[o00]) * dt;
+  const real f2p = (((m00 + A.md[o0p]) * rcp_(r00 + A.rho[o0p])) * A.bt2[o0p]) * dt;
+  const real c1 = f1p - f1, c2 = f2p - f2;
+  real bdv = A.bd[o00];
+  if (A.t2_first) { bdv = bdv + c2; bdv = bdv + c1; }
+  else            { bdv = bdv + c1; bdv = bdv + c2; }
+  A.bdo[o00] = bdv;
+}
+
 // ---------------------------------------------------------------------------------------------
 // c_max reduction, eq (18) PAPER.md:128-132.  c >= 0, and non-negative IEEE doubles order like
 // unsigned integers, so an integer atomicMax on the bit pattern is exact and order independent;

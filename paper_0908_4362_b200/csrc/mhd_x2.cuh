@@ -30,7 +30,11 @@ namespace mhd {
 
 // threads per block (maximum) = shared-memory slot stride: a compile-time constant keeps every exchange
 // address an immediate offset from three base registers (own slot, left and right neighbour)
-template <class real> struct X2Block { static constexpr int NT = sizeof(real) == 4 ? 128 : 256; };
+// NT is also a template parameter of the kernels: rows longer than NT * V cells (512) run in blocks of 2 NT or 4 NT
+// threads (the paper's own 2-D sizes reach 1024^2, Table 2), at proportionally fewer blocks per SM
+template <class real> struct X2Block { static constexpr int NT = sizeof(real) == 4 ? 128 : 256; static constexpr int NT_MAX = sizeof(real) == 4 ? 512 : 512; };
+// blocks per SM for a block of NT threads, given the count tuned for the base block
+template <class real> constexpr int x2_minb(int base, int NT) { return base * X2Block<real>::NT / NT > 0 ? base * X2Block<real>::NT / NT : 1; }
 
 // ---- V-cell vectors of L rows <-> packs ------------------------------------------------------------
 // f2: the two rows arrive as two 16-byte vectors, and a pack must sit in an aligned register PAIR.  ptxas
@@ -340,11 +344,10 @@ __device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const X
 #define MHD_X2_MINB_L(real, T) (sizeof(real) == 8 ? MHD_X2_MINB64 : (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1_L))
 
 // ---- fluid_x --------------------------------------------------------------------------------------
-template <class real, class T>
-__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) fluid_x2_kernel(const XArgs<real> A) {
+template <class real, class T, int NT = X2Block<real>::NT>
+__global__ void __launch_bounds__(NT, x2_minb<real>(MHD_X2_MINB(real, T), NT)) fluid_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
-  constexpr int NT = X2Block<real>::NT;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
@@ -369,11 +372,10 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB(real, T)) fluid
 }
 
 // ---- B_{y->x}, B_{z->x} ------------------------------------------------------------------------------
-template <class real, class T>
-__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB_B(real, T)) bpair_x2_kernel(const XArgs<real> A) {
+template <class real, class T, int NT = X2Block<real>::NT>
+__global__ void __launch_bounds__(NT, x2_minb<real>(MHD_X2_MINB_B(real, T), NT)) bpair_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
-  constexpr int NT = X2Block<real>::NT;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
@@ -405,11 +407,10 @@ __global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB_B(real, T)) bpa
 // ---- reverse L_x in one pass: B_{z->x}, B_{y->x} (t2 first), then fluid_x with the UPDATED field ----
 // Shared memory: 35 slots x NT packs (the B pair uses slots 0..23, the B_x' exchange slot 34,
 // fluid_x slots 0..34; slot 34 is rewritten by fluid_x only two barriers after it was read).
-template <class real, class T>
-__global__ void __launch_bounds__(X2Block<real>::NT, MHD_X2_MINB_L(real, T)) lrev_x2_kernel(const XArgs<real> A) {
+template <class real, class T, int NT = X2Block<real>::NT>
+__global__ void __launch_bounds__(NT, x2_minb<real>(MHD_X2_MINB_L(real, T), NT)) lrev_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
-  constexpr int NT = X2Block<real>::NT;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);

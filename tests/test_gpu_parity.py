@@ -436,7 +436,8 @@ def test_b_pair_ring_march_fp64(B, bring, bc):
 
 @pytest.mark.parametrize("xpack,xfuse", [(1, 0), (1, 1), (2, 0), (2, 1), (3, 1), (3, 3), (2, 2)])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("shape", [(512, 6, 4), (64, 8, 6), (256, 7, 3), (32, 2, 1), (128, 4, 2), (128, 70, 3), (64, 1, 5)])
+@pytest.mark.parametrize("shape", [(512, 6, 4), (64, 8, 6), (256, 7, 3), (32, 2, 1), (128, 4, 2), (128, 70, 3), (64, 1, 5),
+                                   (1024, 4, 2), (640, 3, 2), (2048, 2, 2)])      # rows longer than 512 cells: 2x / 4x blocks
 def test_x_kernels_pack_and_fused_reverse(B, shape, prec, xpack, xfuse):
     """sweeps along x (mhd_x2.cuh): two rows per thread in packed f2 arithmetic (fp32, even ny), and the reverse
     L_x as ONE kernel (B pair, then fluid_x from the updated field), with the fused c_max reduction"""
