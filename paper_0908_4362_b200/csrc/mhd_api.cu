@@ -424,7 +424,11 @@ template <class real>
 static bool x2_ok(const mhd_ctx* c, int kind) {
   constexpr bool f32 = std::is_same<real, float>::value;
   const int V = VecOf<real>::V;
-  if (c->opt_path != 0 || c->bc != MHD_BC_PERIODIC || c->n[0] % V != 0 || c->n[0] / V > X2Block<real>::NT_MAX ||
+  // outflow: one row per thread with 4 clamped ghost cells on either side of the row (mhd_x2.cuh ghost_fix); the fused
+  // reverse L_x does not exist there (its fluid stage would read the B pair's ghost values instead of the clamped outputs)
+  const bool out = c->bc != MHD_BC_PERIODIC;
+  if (out && (kind == 2 || c->n[0] < 8)) return false;
+  if (c->opt_path != 0 || c->n[0] % V != 0 || c->n[0] / V + (out ? 2 * (4 / V) : 0) > X2Block<real>::NT_MAX ||
       c->n[2] > 65535 || c->N >= ((size_t)1 << 31))
     return false;
   // xfuse: 0 never | 1 fp32 only (default; in fp64 the fused kernel is slower than the pair) | 2 always | 3 fp32, packed
@@ -439,12 +443,14 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   // xpack: 1 two rows per thread in packed f2 arithmetic (fp32, even ny) | 2 one row per thread (default) | 3 packed fluid_x only
   // measured at 512^3 fp32: fluid_x one row per thread at six blocks per SM 1.21 ms, packed (two rows per thread,
   // three blocks per SM) 1.23; B pair one row per thread 0.89 ms, packed 1.14: the x kernels want occupancy
-  const bool pack = f32 && c->n[1] % 2 == 0 && c->n[0] / VecOf<real>::V <= X2Block<real>::NT && (c->opt_xpack == 1 || (c->opt_xpack == 3 && kind == 0) || (kind == 2 && c->opt_xfuse == 3));
+  const bool out = c->bc != MHD_BC_PERIODIC;
+  const bool pack = !out && f32 && c->n[1] % 2 == 0 && c->n[0] / VecOf<real>::V <= X2Block<real>::NT && (c->opt_xpack == 1 || (c->opt_xpack == 3 && kind == 0) || (kind == 2 && c->opt_xfuse == 3));
   const int V = VecOf<real>::V, L = pack ? 2 : 1;
   XArgs<real> A;
   memset(&A, 0, sizeof(A));
   A.nx = c->n[0]; A.ny = c->n[1]; A.nz = c->n[2];
-  A.tpr = A.nx / V;
+  A.ghost = out ? 4 / V : 0;
+  A.tpr = A.nx / V + 2 * A.ghost;
   A.tpr_shift = -1;
   for (int b = 0; b < 11; ++b) if ((1 << b) == A.tpr) A.tpr_shift = b;
   // block size: the smallest of NT, 2 NT, 4 NT threads that holds a whole row (packed variants: NT only)
@@ -467,6 +473,10 @@ static int launch_x2(mhd_ctx* c, int kind, int t2_first, bool want_cmax) {
   const size_t slots = kind == 1 ? 24 : 35;
   if (pack) {
     if constexpr (f32) k = kind == 0 ? fluid_x2_kernel<real, T2> : (kind == 1 ? bpair_x2_kernel<real, T2> : lrev_x2_kernel<real, T2>);
+  } else if (out) {
+    if (NT == NT0) k = kind == 0 ? fluid_x2_kernel<real, real, NT0, true> : bpair_x2_kernel<real, real, NT0, true>;
+    else if (NT == 2 * NT0) k = kind == 0 ? fluid_x2_kernel<real, real, 2 * NT0, true> : bpair_x2_kernel<real, real, 2 * NT0, true>;
+    else if constexpr (4 * NT0 <= X2Block<real>::NT_MAX) k = kind == 0 ? fluid_x2_kernel<real, real, 4 * NT0, true> : bpair_x2_kernel<real, real, 4 * NT0, true>;
   } else if (NT == NT0) {
     k = kind == 0 ? fluid_x2_kernel<real, real> : (kind == 1 ? bpair_x2_kernel<real, real> : lrev_x2_kernel<real, real>);
   } else if (NT == 2 * NT0) {

@@ -43,6 +43,7 @@ struct XArgs {
   int tpr_shift;           // log2(tpr) if tpr is a power of two, else -1
   int rpb;                 // row groups per block
   int t2_first;
+  int ghost;               // outflow along x: ghost threads on either side of a row (4 clamped cells), else 0; tpr counts them
   real gamma;
   real one;                // 1.0 at run time (xload)
 };

@@ -78,10 +78,23 @@ struct XRows {
   int o[4];                 // offsets of rows j-1, j, j+1, j+2 of plane k (j+2 only used for L = 2)
   int okm[2], okp[2];       // rows j, j+1 of planes k-1 and k+1
   int onext[2];             // B_x face of the next thread's first column, rows j and j+1
+  int mode;                 // outflow kernels: 0 interior thread, 1 left ghost (every cell = column 0), 2 right ghost (column nx-1)
   bool live;
 };
 
-template <class real, int L>
+// Outflow along x (reading R9: every out-of-range read of an operator INPUT is clamped, intermediates at ghost positions
+// are computed from the clamped inputs): a row group is widened by A.ghost threads = 4 cells on either side whose loads
+// return the edge column and whose results are not stored.  A kept cell depends on inputs at most 3 (fluid) or 4 (B pair)
+// cells away, all of them true ghost values; what the ring of the exchange joins beyond them (the other end's ghosts) never
+// reaches it.
+template <int V, class T>
+__device__ __forceinline__ void ghost_fix(T (&v)[V], int mode) {     // selects, no branch: the edge warps stay in step
+  const T lo = v[0], hi = v[V - 1];
+#pragma unroll
+  for (int i = 0; i < V; ++i) v[i] = mode == 1 ? lo : (mode == 2 ? hi : v[i]);
+}
+
+template <class real, int L, bool OUT = false>
 __device__ __forceinline__ XRows x_rows(const XArgs<real>& A) {
   constexpr int V = VecOf<real>::V;
   XRows r;
@@ -93,17 +106,30 @@ __device__ __forceinline__ XRows x_rows(const XArgs<real>& A) {
   r.live = g < gpp;
   if (!r.live) g = gpp - 1;                           // keep the thread in step for the barriers
   const int k = blockIdx.y, j = g * L;
-  const int kp = (k + 1 == A.nz) ? 0 : k + 1, km = (k == 0) ? A.nz - 1 : k - 1;
-  r.col = r.t * V;
+  r.mode = 0;
+  int kp, km, jm, j1, j2, i_next;
+  if (OUT) {
+    int col = (r.t - A.ghost) * V;
+    if (col < 0) { r.mode = 1; col = 0; }
+    else if (col >= A.nx) { r.mode = 2; col = A.nx - V; }
+    r.col = col;
+    kp = min(k + 1, A.nz - 1); km = max(k - 1, 0);
+    jm = max(j - 1, 0); j1 = min(j + 1, A.ny - 1); j2 = min(j1 + 1, A.ny - 1);
+    i_next = r.mode == 1 ? 0 : (r.mode == 2 ? A.nx - 1 : min(col + V, A.nx - 1));
+    r.live = r.live && r.mode == 0;
+  } else {
+    r.col = r.t * V;
+    kp = (k + 1 == A.nz) ? 0 : k + 1; km = (k == 0) ? A.nz - 1 : k - 1;
+    jm = (j == 0) ? A.ny - 1 : j - 1;
+    j1 = (j + 1 == A.ny) ? 0 : j + 1;                 // L = 2: j is even and ny is even, so j1 = j + 1
+    j2 = (j1 + 1 == A.ny) ? 0 : j1 + 1;
+    i_next = (r.t == A.tpr - 1) ? 0 : (r.t + 1) * V;
+  }
   auto row = [&](int jj, int kk) { return (kk * A.ny + jj) * A.nx + r.col; };
-  const int jm = (j == 0) ? A.ny - 1 : j - 1;
-  const int j1 = (j + 1 == A.ny) ? 0 : j + 1;         // L = 2: j is even and ny is even, so j1 = j + 1
-  const int j2 = (j1 + 1 == A.ny) ? 0 : j1 + 1;
   r.o[0] = row(jm, k); r.o[1] = row(j, k); r.o[2] = row(j1, k); r.o[3] = row(j2, k);
   const int jb = (L == 2) ? j1 : j;
   r.okm[0] = row(j, km); r.okm[1] = row(jb, km);
   r.okp[0] = row(j, kp); r.okp[1] = row(jb, kp);
-  const int i_next = (r.t == A.tpr - 1) ? 0 : (r.t + 1) * V;
   r.onext[0] = (k * A.ny + j) * A.nx + i_next;
   r.onext[1] = (k * A.ny + jb) * A.nx + i_next;
   r.tl = lr * A.tpr + (r.t == 0 ? A.tpr - 1 : r.t - 1);
@@ -267,27 +293,33 @@ __device__ __forceinline__ void bpair_x_core(T* sm, int tid, int tl, int tr, con
 
 // face velocities and transverse fields of the four flux rows of one thread (Alg. 2 step 4, reading R5:
 // momentum sum over density sum of the two cells sharing the face).  r0, m0: rho, m_x of the thread's own cells.
-template <class real, class T, int V>
+template <class real, class T, int V, bool OUT = false>
 __device__ __forceinline__ void bpair_x_inputs(const XArgs<real>& A, const XRows& q, T (&r0)[V], T (&m0)[V],
                                                T (&vt)[4][V], T (&b)[4][V]) {
   T r[V], m[V];
-  xload(A.u[0], q.o[1], q.o[2], r0, A.one); xload(A.u[1], q.o[1], q.o[2], m0, A.one);
-  xload(A.u[0], q.o[0], q.o[1], r, A.one); xload(A.u[1], q.o[0], q.o[1], m, A.one);                  // rows j-1 (, j)
+  auto ld = [&](const real* f, int oa, int ob, T (&v)[V]) { xload(f, oa, ob, v, A.one); };
+  ld(A.u[0], q.o[1], q.o[2], r0); ld(A.u[1], q.o[1], q.o[2], m0);
+  ld(A.u[0], q.o[0], q.o[1], r); ld(A.u[1], q.o[0], q.o[1], m);                  // rows j-1 (, j)
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[0][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
-  xload(A.u[0], q.o[2], q.o[3], r, A.one); xload(A.u[1], q.o[2], q.o[3], m, A.one);                  // rows j+1 (, j+2)
+  ld(A.u[0], q.o[2], q.o[3], r); ld(A.u[1], q.o[2], q.o[3], m);                  // rows j+1 (, j+2)
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[1][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
-  xload(A.u[0], q.okm[0], q.okm[1], r, A.one); xload(A.u[1], q.okm[0], q.okm[1], m, A.one);
+  ld(A.u[0], q.okm[0], q.okm[1], r); ld(A.u[1], q.okm[0], q.okm[1], m);
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[2][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
-  xload(A.u[0], q.okp[0], q.okp[1], r, A.one); xload(A.u[1], q.okp[0], q.okp[1], m, A.one);
+  ld(A.u[0], q.okp[0], q.okp[1], r); ld(A.u[1], q.okp[0], q.okp[1], m);
 #pragma unroll
   for (int v = 0; v < V; ++v) vt[3][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
-  xload(A.by, q.o[1], q.o[2], b[0], A.one);
-  xload(A.by, q.o[2], q.o[3], b[1], A.one);
-  xload(A.bz, q.o[1], q.o[2], b[2], A.one);
-  xload(A.bz, q.okp[0], q.okp[1], b[3], A.one);
+  ld(A.by, q.o[1], q.o[2], b[0]);
+  ld(A.by, q.o[2], q.o[3], b[1]);
+  ld(A.bz, q.o[1], q.o[2], b[2]);
+  ld(A.bz, q.okp[0], q.okp[1], b[3]);
+  if (OUT) {      // ghost threads: every cell is the edge column.  vt is computed column by column, so fixing the results is
+                  // the same as fixing the loads, and it leaves the loads free to be issued back to back
+#pragma unroll
+    for (int p = 0; p < 4; ++p) { ghost_fix<V>(vt[p], q.mode); ghost_fix<V>(b[p], q.mode); }
+  }
 }
 
 // cell-centred field of my V cells from face values (eq (19))
@@ -344,14 +376,15 @@ __device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const X
 #define MHD_X2_MINB_L(real, T) (sizeof(real) == 8 ? MHD_X2_MINB64 : (PackOf<T>::L == 2 ? MHD_X2_MINB2 : MHD_X2_MINB1_L))
 
 // ---- fluid_x --------------------------------------------------------------------------------------
-template <class real, class T, int NT = X2Block<real>::NT>
+// OUT: outflow boundaries (ghost threads, see ghost_fix); one row per thread only
+template <class real, class T, int NT = X2Block<real>::NT, bool OUT = false>
 __global__ void __launch_bounds__(NT, x2_minb<real>(MHD_X2_MINB(real, T), NT)) fluid_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
-  const XRows q = x_rows<real, L>(A);
+  const XRows q = x_rows<real, L, OUT>(A);
   const S dts = (S)(*A.dt);
   const T hdt(S(0.5) * dts), qdt(S(0.25) * dts), gamma(A.gamma);
   T u[5][V];
@@ -361,9 +394,14 @@ __global__ void __launch_bounds__(NT, x2_minb<real>(MHD_X2_MINB(real, T), NT)) f
   xload(A.bx, q.o[1], q.o[2], bxf, A.one);
   xload(A.by, q.o[1], q.o[2], bya, A.one); xload(A.by, q.o[2], q.o[3], byb, A.one);
   xload(A.bz, q.o[1], q.o[2], bza, A.one); xload(A.bz, q.okp[0], q.okp[1], bzb, A.one);
+  bxe[V] = xload1(A.bx, q.onext[0], q.onext[1], (T*)nullptr);
+  if (OUT) {          // after ALL loads are issued (a fix behind each load keeps only two or three of them in flight)
+#pragma unroll
+    for (int c = 0; c < 5; ++c) ghost_fix<V>(u[c], q.mode);
+    ghost_fix<V>(bxf, q.mode); ghost_fix<V>(bya, q.mode); ghost_fix<V>(byb, q.mode); ghost_fix<V>(bza, q.mode); ghost_fix<V>(bzb, q.mode);
+  }
 #pragma unroll
   for (int v = 0; v < V; ++v) bxe[v] = bxf[v];
-  bxe[V] = xload1(A.bx, q.onext[0], q.onext[1], (T*)nullptr);
   BCell<T> B[V];
   x_centre<T, V>(bxe, bya, byb, bza, bzb, B);
   T un[V][5];
@@ -372,18 +410,18 @@ __global__ void __launch_bounds__(NT, x2_minb<real>(MHD_X2_MINB(real, T), NT)) f
 }
 
 // ---- B_{y->x}, B_{z->x} ------------------------------------------------------------------------------
-template <class real, class T, int NT = X2Block<real>::NT>
+template <class real, class T, int NT = X2Block<real>::NT, bool OUT = false>
 __global__ void __launch_bounds__(NT, x2_minb<real>(MHD_X2_MINB_B(real, T), NT)) bpair_x2_kernel(const XArgs<real> A) {
   constexpr int V = VecOf<real>::V;
   constexpr int L = PackOf<T>::L;
   typedef typename PackOf<T>::scalar S;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sm = reinterpret_cast<T*>(smem_raw);
-  const XRows q = x_rows<real, L>(A);
+  const XRows q = x_rows<real, L, OUT>(A);
   const S dts = (S)(*A.dt);
   const T dt(dts), hdt(S(0.5) * dts);
   T r0[V], m0[V], vt[4][V], b[4][V], f[4][V + 1];
-  bpair_x_inputs<real, T, V>(A, q, r0, m0, vt, b);
+  bpair_x_inputs<real, T, V, OUT>(A, q, r0, m0, vt, b);
   bpair_x_core<T, V, NT>(sm, threadIdx.x, q.tl, q.tr, vt, b, dt, hdt, f);
   // advect B_y, B_z (Alg. 2 step 9) and constrain B_x with the same fluxes
   T bxv[V], byn[V], bzn[V];

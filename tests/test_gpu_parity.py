@@ -384,6 +384,44 @@ def test_packed_fp32_kernels(B, nx, bc):
             assert abs(cmg - cm) <= 2e-6 * cm, (pack, bc, seg, s0, cmg, cm)
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(512, 6, 4), (1016, 3, 2), (1024, 4, 2), (2040, 2, 2), (8, 5, 3), (256, 1, 1)])
+def test_x_kernels_outflow(B, shape, prec):
+    """sweeps along x with outflow boundaries on the specialised kernels (mhd_x2.cuh, ghost threads: four clamped cells on
+    either side of a row, reading R9), rows of every block size: fluid_x, the B pair in both orders, a forward and a
+    reverse sweep, and a whole step with the fused c_max reduction, element-wise against the oracle"""
+    nx, ny, nz = shape
+    f0 = random_state(nx, ny, nz, seed=411 + nx + ny)
+    gamma, dt = 5.0 / 3.0, 0.2
+    tol = TOL64 if prec == "f64" else TOL32_STEP
+    for op, rev in [(B.MHD_OP_FLUID, 0), (B.MHD_OP_BPAIR, 0), (B.MHD_OP_BPAIR, 1),
+                    (B.MHD_OP_SWEEP_FORWARD, 0), (B.MHD_OP_SWEEP_REVERSE, 0)]:
+        ref = _ref_input(f0, prec)
+        if op == B.MHD_OP_FLUID:
+            oracle.fluid(ref, gamma, O, 0, dt)
+        elif op == B.MHD_OP_BPAIR:
+            for t in ((2, 1) if rev else (1, 2)):
+                oracle.badvect(ref, gamma, O, 0, t, dt)
+        else:
+            oracle.sweep(ref, gamma, O, 0, op == B.MHD_OP_SWEEP_REVERSE, dt)
+        s = _solver(B, f0, gamma, O, prec)
+        s.apply(op, 0, rev, dt)
+        got = s.get_state()
+        s.close()
+        e = max_rel(got, ref)
+        assert worst(e) <= tol, (shape, prec, op, rev, e)
+    ref = _ref_input(f0, prec)
+    oracle.step_fixed(ref, gamma, O, 0, dt)
+    s = _solver(B, f0, gamma, O, prec)
+    s.step_fixed(1, dt)
+    got = s.get_state()
+    _, cmg = s.cfl_dt(0.8)
+    s.close()
+    assert worst(max_rel(got, ref)) <= tol
+    cm = oracle.cmax([np.array(a, dtype=np.float64) for a in got], gamma, O)
+    assert abs(cmg - cm) <= (1e-13 if prec == "f64" else 2e-6) * cm
+
+
 @pytest.mark.parametrize("shape", [(256, 14, 20), (512, 6, 10), (256, 2, 2), (768, 4, 12), (128, 10, 12), (384, 8, 6)])
 @pytest.mark.parametrize("bc", [P, O])
 def test_b_pair_two_rows_per_thread(B, shape, bc):
