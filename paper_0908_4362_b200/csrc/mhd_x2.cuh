@@ -20,8 +20,9 @@
 //    The FORWARD operator cannot be fused this way: its B pair needs the UPDATED rho, m_x of the four
 //    transverse neighbour rows, i.e. the fluid update of rows this block does not own.
 //
-// Requirements (else the generic kernels of mhd_generic.cuh run): periodic BC, nx % V == 0,
-// nx / V <= 256, N < 2^31, and for T = f2 an even ny.
+// Requirements (else the generic kernels of mhd_generic.cuh run): nx % V == 0, a row (plus its ghost threads under
+// outflow boundaries, see ghost_fix) within 512 threads, i.e. nx <= 2048 (fp32) / 1024 (fp64), N < 2^31; the packed (f2)
+// and fused variants additionally need periodic boundaries, nx <= 512 and (f2) an even ny.
 #pragma once
 #include "mhd_args.cuh"
 #include "mhd_pack_io.cuh"
