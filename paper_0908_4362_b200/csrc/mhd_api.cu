@@ -289,10 +289,14 @@ static void swap_fields(mhd_ctx* c, const int* f, int n) {
 static const int kBFields[3] = {5, 6, 7};
 
 // ---- ring marches for sweeps along y and z (mhd_yz2.cuh, mhd_bring.cuh) ------------------------
-// tile width in columns: fp32 256 (128 threads, two pencils each) when nx allows, else 128; fp64 128
+// tile width in columns: fp32 256 (128 threads, two pencils each) or 128, fp64 128; the last tile of a row may be narrower
+// (rows must be a multiple of 16 bytes for the bulk copies), so the width that wastes fewer lanes is taken
 static int yz_tile(const mhd_ctx* c) {
-  if (c->precision == MHD_F32 && c->n[0] % 256 == 0) return 256;
-  return c->n[0] % 128 == 0 ? 128 : 0;
+  const int nx = c->n[0], ch = c->precision == MHD_F32 ? 4 : 2;
+  if (nx % ch != 0) return 0;
+  if (c->precision != MHD_F32) return 128;
+  const double e256 = (double)nx / (((nx + 255) / 256) * 256), e128 = (double)nx / (((nx + 127) / 128) * 128);
+  return e256 + 0.02 >= e128 ? 256 : 128;
 }
 
 static bool yz_ok(const mhd_ctx* c, int d) {
@@ -327,7 +331,7 @@ static YZArgs<real> make_yz(mhd_ctx* c, int d, int tile, int blocks_per_sm, int 
   A.gamma = (real)c->gamma;
   A.dt = &c->sc->dt;
   int seg = c->opt_segment;
-  if (seg < 0) seg = pick_segment(A.nd, ((long long)A.nx / tile) * A.no, (long long)c->sm_count * blocks_per_sm, halo);
+  if (seg < 0) seg = pick_segment(A.nd, (long long)((A.nx + tile - 1) / tile) * A.no, (long long)c->sm_count * blocks_per_sm, halo);
   if (seg == 0 || seg > A.nd) seg = A.nd;
   A.seg = seg;
   return A;
@@ -348,7 +352,7 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
   A.src[5] = (const char*)A.bd - (const char*)A.u[0];
   A.src[6] = (const char*)A.bo - (const char*)A.u[0];
   A.src[7] = (const char*)A.bx - (const char*)A.u[0];
-  const dim3 grid(A.nx / P, A.no, (A.nd + A.seg - 1) / A.seg);
+  const dim3 grid((A.nx + P - 1) / P, A.no, (A.nd + A.seg - 1) / A.seg);
   void (*k)(const YZArgs<real>) = nullptr;
   size_t smem = 0;
   constexpr int DR = MHD_YZ2_STAGES;
@@ -384,7 +388,7 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   YZArgs<real> A = make_yz<real>(c, d, W, two ? 2 : MHD_BRING_MINB, 8);
   if (two) {                                   // a block covers two rows: half as many pencil blocks
     int seg = c->opt_segment;
-    if (seg < 0) seg = pick_segment(A.nd, ((long long)A.nx / W) * (A.no / 2), (long long)c->sm_count * (W == 256 ? 2 : 4), 8);
+    if (seg < 0) seg = pick_segment(A.nd, (long long)((A.nx + W - 1) / W) * (A.no / 2), (long long)c->sm_count * (W == 256 ? 2 : 4), 8);
     if (seg == 0 || seg > A.nd) seg = A.nd;
     A.seg = seg;
   }
@@ -397,7 +401,7 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   A.src[5] = (const char*)A.bd - (const char*)A.u[0];
   A.src[6] = (const char*)A.bo - (const char*)A.u[0];
   A.src[7] = (const char*)A.bx - (const char*)A.u[0];
-  const dim3 grid(A.nx / W, two ? A.no / 2 : A.no, (A.nd + A.seg - 1) / A.seg);
+  const dim3 grid((A.nx + W - 1) / W, two ? A.no / 2 : A.no, (A.nd + A.seg - 1) / A.seg);
   constexpr int D = MHD_BRING_STAGES;
   void (*k)(const YZArgs<real>) = nullptr;
   size_t smem = 0;

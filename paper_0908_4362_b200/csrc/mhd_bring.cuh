@@ -19,7 +19,8 @@
 // (ncu on a first version that re-read B_t(k-4) from the ring and so kept stages four steps longer showed
 // the consumers waiting on the full-barriers: 4 stages in flight do not cover the HBM latency).
 //
-// Requirements (else bpair_march_kernel of mhd_generic.cuh runs): nx % TXB == 0, extent along d >= 8.
+// Requirements (else bpair_march_kernel of mhd_generic.cuh runs): nx a multiple of 16 bytes (a narrower last tile per row
+// is allowed, as in mhd_yz2.cuh), extent along d >= 8.
 #pragma once
 #include <type_traits>
 #include "mhd_args.cuh"
@@ -73,10 +74,11 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // the same value, warp-uniform for the compiler too
   const int x0 = blockIdx.x * TXB, o = blockIdx.y;
+  const int w = min(TXB, A.nx - x0);                      // columns of this tile
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
   const int niter = (n1 - n0 + 8 + 3) & ~3;               // cells n0-4 .. n1+3, rounded up to the 4x unrolled march
-  const int xl = map_index1(x0 - 1, A.nx, A.bc), xr = map_index1(x0 + TXB, A.nx, A.bc);
+  const int xl = map_index1(x0 - 1, A.nx, A.bc), xr = map_index1(x0 + w, A.nx, A.bc);
   if (tid == 0) {
     for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
     mbar_fence_init();
@@ -108,10 +110,10 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
 #endif
       real* st = ring + s * RG::STAGE;
       uint64_t* bar = &full[s];
-      constexpr uint32_t RB = TXB * sizeof(real);
+      const uint32_t RB = (uint32_t)w * sizeof(real);
       const char* rho = reinterpret_cast<const char*>(A.u[0] + od);
       const char* md = rho + A.src[1];
-      mbar_expect_tx(bar, RG::BYTES);
+      mbar_expect_tx(bar, (uint32_t)RG::ROWS * RB + RG::NCHUNK * 16u);
       bulk_g2s(st + 0 * P + CH, rho + om_b, RB, bar);
       bulk_g2s(st + 1 * P + CH, rho + o_b, RB, bar);
       bulk_g2s(st + 2 * P + CH, rho + op_b, RB, bar);
@@ -123,10 +125,10 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
       bulk_g2s(st + 8 * P + CH, rho + A.src[6] + op_b, RB, bar);
       bulk_g2s(st + 9 * P + CH, reinterpret_cast<const char*>(A.u[0] + odl) + A.src[5] + o_b, RB, bar);
       bulk_g2s(st + 1 * P, rho + cl_b, 16, bar);
-      bulk_g2s(st + 1 * P + CH + TXB, rho + cr_b, 16, bar);
+      bulk_g2s(st + 1 * P + CH + w, rho + cr_b, 16, bar);
       bulk_g2s(st + 4 * P, md + cl_b, 16, bar);
-      bulk_g2s(st + 4 * P + CH + TXB, md + cr_b, 16, bar);
-      bulk_g2s(st + 6 * P + CH + TXB, rho + A.src[7] + cr_b, 16, bar);
+      bulk_g2s(st + 4 * P + CH + w, md + cr_b, 16, bar);
+      bulk_g2s(st + 6 * P + CH + w, rho + A.src[7] + cr_b, 16, bar);
     }
     __syncwarp();
   };
@@ -136,7 +138,8 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   typedef typename PackOf<T>::scalar S;
   const int cx = CH + L * tid;                            // my first column inside a stage row
   const int iL = tid == 0 ? xl % CH : cx - 1;             // column to my left / right (the chunks at the row ends)
-  const int iR = tid == NC - 1 ? CH + TXB + xr % CH : cx + L;
+  const int iR = L * tid + L == w ? CH + w + xr % CH : cx + L;
+  const bool active = L * tid < w;                        // threads beyond a narrow last tile store nothing
   const S dts = (S)(*A.dt);
   const T dt(dts), hdt(S(0.5) * dts);
   const bool x_first = (A.x_is_t1 != 0) != (A.t2_first != 0);     // forward: t1 then t2; reverse: t2 then t1
@@ -176,7 +179,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
     po.template push<K>(vtO, bo, dt, hdt, bon, folo);
     pop.template push<K>(vtP, bop, dt, hdt, bpn, fplo);
     const int m = n0 + it - 8;
-    if (it >= 8 && m < n1) {
+    if (it >= 8 && m < n1 && active) {
       st_pack(A.bxo + off, bxn);                            // Alg. 2 step 9: advected B_t
       st_pack(A.boo + off, bon);
       // constraint with the same fluxes at face m-1/2: rows x+1 and o+1
@@ -244,10 +247,11 @@ __global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kerne
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int x0 = blockIdx.x * TXB, o = 2 * blockIdx.y;
+  const int w = min(TXB, A.nx - x0);
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
   const int niter = (n1 - n0 + 8 + 3) & ~3;
-  const int xl = map_index1(x0 - 1, A.nx, A.bc), xr = map_index1(x0 + TXB, A.nx, A.bc);
+  const int xl = map_index1(x0 - 1, A.nx, A.bc), xr = map_index1(x0 + w, A.nx, A.bc);
   if (tid == 0) {
     for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
     mbar_fence_init();
@@ -266,13 +270,13 @@ __global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kerne
       const int odl = map_index1(n0 - 8 + itp, A.nd, A.bc) * A.sd;
       real* st = ring + s * RG::STAGE;
       uint64_t* bar = &full[s];
-      constexpr uint32_t RB = TXB * sizeof(real);
+      const uint32_t RB = (uint32_t)w * sizeof(real);
       const char* rho = reinterpret_cast<const char*>(A.u[0] + od);
       const char* md = rho + A.src[1];
       const char* bx = rho + A.src[7];
       const char* bo = rho + A.src[6];
       const char* bd = reinterpret_cast<const char*>(A.u[0] + odl) + A.src[5];
-      mbar_expect_tx(bar, RG::BYTES);
+      mbar_expect_tx(bar, (uint32_t)RG::ROWS * RB + RG::NCHUNK * 16u);
       bulk_g2s(st + 0 * P + CH, rho + om_b, RB, bar);
       bulk_g2s(st + 1 * P + CH, rho + o_b, RB, bar);
       bulk_g2s(st + 2 * P + CH, rho + o1_b, RB, bar);
@@ -289,15 +293,15 @@ __global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kerne
       bulk_g2s(st + 13 * P + CH, bd + o_b, RB, bar);
       bulk_g2s(st + 14 * P + CH, bd + o1_b, RB, bar);
       bulk_g2s(st + 1 * P, rho + o_b + cl_b, 16, bar);
-      bulk_g2s(st + 1 * P + CH + TXB, rho + o_b + cr_b, 16, bar);
+      bulk_g2s(st + 1 * P + CH + w, rho + o_b + cr_b, 16, bar);
       bulk_g2s(st + 2 * P, rho + o1_b + cl_b, 16, bar);
-      bulk_g2s(st + 2 * P + CH + TXB, rho + o1_b + cr_b, 16, bar);
+      bulk_g2s(st + 2 * P + CH + w, rho + o1_b + cr_b, 16, bar);
       bulk_g2s(st + 5 * P, md + o_b + cl_b, 16, bar);
-      bulk_g2s(st + 5 * P + CH + TXB, md + o_b + cr_b, 16, bar);
+      bulk_g2s(st + 5 * P + CH + w, md + o_b + cr_b, 16, bar);
       bulk_g2s(st + 6 * P, md + o1_b + cl_b, 16, bar);
-      bulk_g2s(st + 6 * P + CH + TXB, md + o1_b + cr_b, 16, bar);
-      bulk_g2s(st + 8 * P + CH + TXB, bx + o_b + cr_b, 16, bar);
-      bulk_g2s(st + 9 * P + CH + TXB, bx + o1_b + cr_b, 16, bar);
+      bulk_g2s(st + 6 * P + CH + w, md + o1_b + cr_b, 16, bar);
+      bulk_g2s(st + 8 * P + CH + w, bx + o_b + cr_b, 16, bar);
+      bulk_g2s(st + 9 * P + CH + w, bx + o1_b + cr_b, 16, bar);
     }
     __syncwarp();
   };
@@ -305,7 +309,8 @@ __global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kerne
 
   const int cx = CH + L * tid;
   const int iL = tid == 0 ? xl % CH : cx - 1;
-  const int iR = tid == NC - 1 ? CH + TXB + xr % CH : cx + L;
+  const int iR = L * tid + L == w ? CH + w + xr % CH : cx + L;
+  const bool active = L * tid < w;
   const S dts = (S)(*A.dt);
   const T dt(dts), hdt(S(0.5) * dts);
   const bool x_first = (A.x_is_t1 != 0) != (A.t2_first != 0);
@@ -348,7 +353,7 @@ __global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kerne
     po1.template push<K>(vtO1, bo1, dt, hdt, bon1, fo1);
     po2.template push<K>(vtO2, bo2, dt, hdt, bon2, fo2);
     const int m = n0 + it - 8;
-    if (it >= 8 && m < n1) {
+    if (it >= 8 && m < n1 && active) {
       st_pack(A.bxo + off, bxn0);                           // Alg. 2 step 9: advected B_t, rows o and o+1
       st_pack(A.boo + off, bon0);
       st_pack(A.bxo + off + A.so, bxn1);

@@ -17,7 +17,9 @@
 //     instructions per step, and five-warp blocks leave one scheduler with three warps, which caps
 //     every thread at 168 registers.
 //
-// Requirements (else fluid_march_kernel of mhd_generic.cuh runs): nx % TXB == 0, extent along the sweep >= 8.
+// Requirements (else fluid_march_kernel of mhd_generic.cuh runs): nx a multiple of 16 bytes (the last tile of a row may be
+// narrower than TXB: its copies are shorter and the threads beyond it compute on stale shared memory and store nothing),
+// extent along the sweep >= 8.
 #pragma once
 #include "mhd_args.cuh"
 #include "mhd_async.cuh"
@@ -80,6 +82,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // the same value, warp-uniform for the compiler too
   const int x0 = blockIdx.x * TXB;
+  const int w = min(TXB, A.nx - x0);                     // columns of this tile (a multiple of the 16-byte chunk)
   const int o = blockIdx.y;
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
@@ -98,7 +101,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   const int rowbase = x0 + o * A.so;
 #endif
   const long long op_bytes = (long long)((map_index1(o + 1, A.no, A.bc) - o) * A.so) * (long long)sizeof(real);
-  const long long xc_bytes = (long long)((map_index1(x0 + TXB, A.nx, A.bc) / RG::CH) * RG::CH - x0) * (long long)sizeof(real);   // B_x at x0+TXB lives in this 16-byte chunk
+  const long long xc_bytes = (long long)((map_index1(x0 + w, A.nx, A.bc) / RG::CH) * RG::CH - x0) * (long long)sizeof(real);   // B_x at x0+w lives in this 16-byte chunk
   auto produce = [&](int itp) {                          // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
 #ifndef MHD_BUG_NO_EMPTY_WAIT        // (fault injection for tests/test_gpu_jitter.py: refill a stage without waiting for its readers)
@@ -116,8 +119,8 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
       const char* b0 = reinterpret_cast<const char*>(A.u[0] + od + rowbase);     // row (q, o), columns x0.. of field u[0]
       const char* b1 = reinterpret_cast<const char*>(A.u[0] + od1 + rowbase);    // row (q+1, o)
       real* st = ring + s * RG::STAGE;
-      constexpr uint32_t RB = TXB * sizeof(real);
-      mbar_expect_tx(&full[s], RG::BYTES);
+      const uint32_t RB = (uint32_t)w * sizeof(real);
+      mbar_expect_tx(&full[s], 9u * RB + 16u);
 #pragma unroll
       for (int k = 0; k < 5; ++k) bulk_g2s(st + k * RG::ROW, b0 + A.src[k], RB, &full[s]);
       bulk_g2s(st + 5 * RG::ROW, b1 + A.src[5], RB, &full[s]);               // B_d at the next face
@@ -134,13 +137,14 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   const int c2 = L * tid;
   const S dts = (S)(*A.dt);
   const T hdt(S(0.5) * dts), qdt(S(0.25) * dts), gamma(A.gamma);
-  const int xn = map_index1(x0 + TXB, A.nx, A.bc);
-  const int xp_idx = 8 * RG::ROW + (c2 + L < TXB ? L : TXB - c2 + (xn % RG::CH));   // B_x at column c2+L, relative to my column
+  const int xn = map_index1(x0 + w, A.nx, A.bc);
+  const int xp_idx = 8 * RG::ROW + (c2 + L < w ? L : TXB - c2 + (xn % RG::CH));   // B_x at column c2+L, relative to my column
+  const bool active = c2 < w;                            // threads beyond a narrow last tile store nothing
   T* tag = nullptr;
 
   FluidPipe<T> pipe;
   pipe.init();
-  T bd_lo = ld_pack(A.bd + map_index1(n0 - 3, A.nd, A.bc) * A.sd + x0 + c2 + o * A.so, tag);
+  T bd_lo = ld_pack(A.bd + map_index1(n0 - 3, A.nd, A.bc) * A.sd + x0 + (active ? c2 : 0) + o * A.so, tag);
   decltype(pack_speed_key((const T*)nullptr, T(), S())) cbest = 0;
   // ring slots of the current group of four march steps and of the previous one (D = 8: the two halves of the ring),
   // as this thread's column inside stage 0 of each half; barrier addresses likewise
@@ -187,7 +191,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
     bd_lo = bd_hi;
     T out[5];
     pipe.advance(u, um1, um3, B, gamma, hdt, qdt, out);
-    if (it >= 6 && it - 6 < n1 - n0) {                   // cell q-3 = n0 - 6 + it
+    if (it >= 6 && it - 6 < n1 - n0 && active) {         // cell q-3 = n0 - 6 + it
 #pragma unroll
       for (int k = 0; k < 5; ++k) st_pack(A.uo[k] + off, out[k]);
       if (CM) {                   // last operator of a step: c of eq (18) from the updated cells (B unchanged)

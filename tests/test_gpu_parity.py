@@ -359,7 +359,7 @@ def test_fused_cfl_reduction_paths(B):
     s.close()
 
 
-@pytest.mark.parametrize("nx", [512, 384, 128])       # 256-wide ring tiles, 128-wide ring tiles, a single tile
+@pytest.mark.parametrize("nx", [512, 384, 128, 320, 200, 72])   # 256-wide ring tiles, 128-wide ring tiles, a single tile, narrower last tiles
 @pytest.mark.parametrize("bc", [P, O])
 def test_packed_fp32_kernels(B, nx, bc):
     """fp32 kernels that advance two pencils per thread in packed f2 arithmetic (mhd_yz2.cuh, mhd_bring.cuh): both tile
@@ -422,7 +422,7 @@ def test_x_kernels_outflow(B, shape, prec):
     assert abs(cmg - cm) <= (1e-13 if prec == "f64" else 2e-6) * cm
 
 
-@pytest.mark.parametrize("shape", [(256, 14, 20), (512, 6, 10), (256, 2, 2), (768, 4, 12), (128, 10, 12), (384, 8, 6)])
+@pytest.mark.parametrize("shape", [(256, 14, 20), (512, 6, 10), (256, 2, 2), (768, 4, 12), (128, 10, 12), (384, 8, 6), (320, 6, 10), (44, 8, 12)])
 @pytest.mark.parametrize("bc", [P, O])
 def test_b_pair_two_rows_per_thread(B, shape, bc):
     """bpair_ring2_kernel (mhd_bring.cuh; option brows = 2): two rows o, o+1 per thread, six packed flux pipelines for four
