@@ -357,17 +357,19 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
   size_t smem = 0;
   constexpr int DR = MHD_YZ2_STAGES;
   const bool xt1 = A.x_is_t1 != 0;
+  const bool rag = A.nx % P != 0;
+#define MHD_FYZ_PICK(TX_, RAG_)                                                                                          \
+  do {                                                                                                                   \
+    smem = FluidRing<real, TX_>::smem_bytes(DR);                                                                         \
+    k = want_cmax ? (xt1 ? fluid_yz_ring_kernel<real, T, TX_, DR, true, true, RAG_> : fluid_yz_ring_kernel<real, T, TX_, DR, false, true, RAG_>) \
+                  : (xt1 ? fluid_yz_ring_kernel<real, T, TX_, DR, true, false, RAG_> : fluid_yz_ring_kernel<real, T, TX_, DR, false, false, RAG_>); \
+  } while (0)
   if (P == 256) {
-    if constexpr (f32) {
-      smem = FluidRing<real, 256>::smem_bytes(DR);
-      k = want_cmax ? (xt1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, true> : fluid_yz_ring_kernel<real, T, 256, DR, false, true>)
-                    : (xt1 ? fluid_yz_ring_kernel<real, T, 256, DR, true, false> : fluid_yz_ring_kernel<real, T, 256, DR, false, false>);
-    }
+    if constexpr (f32) { if (rag) MHD_FYZ_PICK(256, true); else MHD_FYZ_PICK(256, false); }
   } else {
-    smem = FluidRing<real, 128>::smem_bytes(DR);
-    k = want_cmax ? (xt1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, true> : fluid_yz_ring_kernel<real, T, 128, DR, false, true>)
-                  : (xt1 ? fluid_yz_ring_kernel<real, T, 128, DR, true, false> : fluid_yz_ring_kernel<real, T, 128, DR, false, false>);
+    if (rag) MHD_FYZ_PICK(128, true); else MHD_FYZ_PICK(128, false);
   }
+#undef MHD_FYZ_PICK
   int rc = want_smem(c, (const void*)k, smem);
   if (rc) return rc;
   k<<<grid, P / PackOf<T>::L, smem, c->stream>>>(A);
@@ -405,14 +407,15 @@ static int launch_bpair_yz(mhd_ctx* c, int d, int t2_first) {
   constexpr int D = MHD_BRING_STAGES;
   void (*k)(const YZArgs<real>) = nullptr;
   size_t smem = 0;
+  const bool rag = A.nx % W != 0;
   if (two) {
     if constexpr (f32) {
-      if (W == 256) { k = bpair_ring2_kernel<256, MHD_BRING2_STAGES>; smem = BRowRing2<real, 256>::smem_bytes(MHD_BRING2_STAGES); }
-      else          { k = bpair_ring2_kernel<128, MHD_BRING2_STAGES>; smem = BRowRing2<real, 128>::smem_bytes(MHD_BRING2_STAGES); }
+      if (W == 256) { k = rag ? bpair_ring2_kernel<256, MHD_BRING2_STAGES, true> : bpair_ring2_kernel<256, MHD_BRING2_STAGES, false>; smem = BRowRing2<real, 256>::smem_bytes(MHD_BRING2_STAGES); }
+      else          { k = rag ? bpair_ring2_kernel<128, MHD_BRING2_STAGES, true> : bpair_ring2_kernel<128, MHD_BRING2_STAGES, false>; smem = BRowRing2<real, 128>::smem_bytes(MHD_BRING2_STAGES); }
     }
   } else if (W == 256) {
-    if constexpr (f32) { k = bpair_ring_kernel<real, T, 256, D>; smem = BRowRing<real, 256>::smem_bytes(D); }
-  } else { k = bpair_ring_kernel<real, T, 128, D>; smem = BRowRing<real, 128>::smem_bytes(D); }
+    if constexpr (f32) { k = rag ? bpair_ring_kernel<real, T, 256, D, true> : bpair_ring_kernel<real, T, 256, D, false>; smem = BRowRing<real, 256>::smem_bytes(D); }
+  } else { k = rag ? bpair_ring_kernel<real, T, 128, D, true> : bpair_ring_kernel<real, T, 128, D, false>; smem = BRowRing<real, 128>::smem_bytes(D); }
   int rc = want_smem(c, (const void*)k, smem);
   if (rc) return rc;
   k<<<grid, W / PackOf<T>::L, smem, c->stream>>>(A);

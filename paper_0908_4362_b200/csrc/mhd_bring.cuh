@@ -57,7 +57,7 @@ struct BRowRing {
 // real: element type in memory (float/double).  T: arithmetic pack (f2 for float, double for double).
 // No producer warp: the warps take turns (march step modulo the warp count) at issuing the copies of the
 // stage PF steps ahead, one copy per lane (see mhd_yz2.cuh for why).
-template <class real, class T, int TXB, int D>
+template <class real, class T, int TXB, int D, bool RAG = false>
 __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring_kernel(const YZArgs<real> A) {
   using RG = BRowRing<real, TXB>;
   constexpr int L = PackOf<T>::L;
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // the same value, warp-uniform for the compiler too
   const int x0 = blockIdx.x * TXB, o = blockIdx.y;
-  const int w = min(TXB, A.nx - x0);                      // columns of this tile
+  const int w = RAG ? min(TXB, A.nx - x0) : TXB;          // columns of this tile (RAG: the row ends in a narrower one)
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
   const int niter = (n1 - n0 + 8 + 3) & ~3;               // cells n0-4 .. n1+3, rounded up to the 4x unrolled march
@@ -227,7 +227,7 @@ struct BRowRing2 {
 #define MHD_BRING2_SLACK 1
 #endif
 
-template <int TXB, int D>
+template <int TXB, int D, bool RAG = false>
 __global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kernel(const YZArgs<float> A) {
   typedef float real;
   typedef f2 T;
@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(TXB / 2, TXB == 256 ? 2 : 4) bpair_ring2_kerne
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int x0 = blockIdx.x * TXB, o = 2 * blockIdx.y;
-  const int w = min(TXB, A.nx - x0);
+  const int w = RAG ? min(TXB, A.nx - x0) : TXB;
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
   const int niter = (n1 - n0 + 8 + 3) & ~3;

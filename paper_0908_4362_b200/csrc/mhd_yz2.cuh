@@ -65,7 +65,8 @@ struct FluidRing {
 // its ten source rows as  u[0] + (row offset) + A.src[k]  with the byte offsets A.src[] in the constant bank, the
 // consumers keep one running store offset, and the march is unrolled by four with the step number modulo 4 a
 // compile-time constant.
-template <class real, class T, int TXB, int D, bool XT1, bool CM>
+// RAG: the row ends in a tile narrower than TXB (else the width is a compile-time constant, as the tuned kernel wants)
+template <class real, class T, int TXB, int D, bool XT1, bool CM, bool RAG = false>
 __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_ring_kernel(const YZArgs<real> A) {
   using RG = FluidRing<real, TXB>;
   typedef typename PackOf<T>::scalar S;
@@ -82,7 +83,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // the same value, warp-uniform for the compiler too
   const int x0 = blockIdx.x * TXB;
-  const int w = min(TXB, A.nx - x0);                     // columns of this tile (a multiple of the 16-byte chunk)
+  const int w = RAG ? min(TXB, A.nx - x0) : TXB;         // columns of this tile (a multiple of the 16-byte chunk)
   const int o = blockIdx.y;
   const int n0 = blockIdx.z * A.seg;
   const int n1 = min(n0 + A.seg, A.nd);
