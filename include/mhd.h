@@ -172,6 +172,8 @@ int mhd_viz_volume(mhd_ctx* ctx, int field, double vmin, double vmax, const unsi
  *   "block"   threads per block of the generic kernels (multiple of 32 in [32, 256])
  *   "brows"   B pair along y, z in fp32 on 256-column tiles: 2 (default) two rows per thread where the extent along the other
  *             transverse axis is even | 1 one row per thread
+ *   "tmap"    fluid_y / fluid_z ring kernel in fp32 on whole 256-column tiles: 0 (default) 1-D bulk copies | 1 the nine row
+ *             copies of a stage as tensor-map TMA copies (same bits, measured no faster: DESIGN.md section 12)
  *   "xpack"   x kernels: 1 two rows per thread in packed f32x2 arithmetic (fp32, even ny) | 2 one row per thread (default)
  *             | 3 packed fluid_x only
  *   "xfuse"   reverse L_x in one kernel: 0 off | 1 fp32 only (default) | 2 always | 3 fp32, packed

@@ -57,7 +57,11 @@ struct mhd_ctx {
   long long step_index;
   long long launches;
   // options
-  int opt_segment, opt_block, opt_path, opt_xpack, opt_xfuse, opt_brows;
+  int opt_segment, opt_block, opt_path, opt_xpack, opt_xfuse, opt_brows, opt_tmap;
+  // tensor maps of the field buffers (option tmap): one per buffer, box 256 x 1 x 1
+  const void* tmap_ptr[16];
+  CUtensorMap tmap[16];
+  int n_tmap;
   const void* smem_set[48];   // kernels whose dynamic shared-memory limit has been raised on this context's device
   int n_smem_set;
   int opt_fuse;            // fused reverse L_y / L_z and fused middle pair (mhd_lrev.cuh): 0 off, 1 on, 2 middle pair fuses the two B pairs only
@@ -135,6 +139,8 @@ extern "C" int mhd_create(int nx, int ny, int nz, double gamma, int precision, i
   c->opt_xpack = 2;
   c->opt_xfuse = 1;
   c->opt_brows = 2;
+  c->opt_tmap = 0;
+  c->n_tmap = 0;
   c->opt_graph = -1;
   c->opt_cmax_reuse = 1;
   c->opt_fuse = 0;
@@ -337,6 +343,34 @@ static YZArgs<real> make_yz(mhd_ctx* c, int d, int tile, int blocks_per_sm, int 
   return A;
 }
 
+// 3-D tensor map (x, y, z) of one field buffer with a box of `tile` x 1 x 1 elements, cached per buffer.  The driver's
+// encoder is looked up at run time (the library links the static runtime only).
+static int get_tmap(mhd_ctx* c, const void* ptr, int tile, CUtensorMap* out) {
+  for (int i = 0; i < c->n_tmap; ++i)
+    if (c->tmap_ptr[i] == ptr) { *out = c->tmap[i]; return MHD_OK; }
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn enc = nullptr;
+  if (!enc) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    CUDA_TRY(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+    if (!fn || q != cudaDriverEntryPointSuccess) return fail(c, MHD_ECUDA, "cuTensorMapEncodeTiled is not available");
+    enc = (encode_fn)fn;
+  }
+  const cuuint64_t dims[3] = {(cuuint64_t)c->n[0], (cuuint64_t)c->n[1], (cuuint64_t)c->n[2]};
+  const cuuint64_t strides[2] = {(cuuint64_t)c->n[0] * c->esize, (cuuint64_t)c->n[0] * c->n[1] * c->esize};
+  const cuuint32_t box[3] = {(cuuint32_t)tile, 1, 1}, estr[3] = {1, 1, 1};
+  alignas(64) CUtensorMap m;
+  const CUresult r = enc(&m, c->precision == MHD_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(ptr),
+                         dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(c, MHD_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  if (c->n_tmap < 16) { c->tmap_ptr[c->n_tmap] = ptr; c->tmap[c->n_tmap] = m; c->n_tmap++; }
+  *out = m;
+  return MHD_OK;
+}
+
 template <class real>
 static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
   constexpr bool f32 = std::is_same<real, float>::value;
@@ -370,6 +404,24 @@ static int launch_fluid_yz(mhd_ctx* c, int d, bool want_cmax) {
     if (rag) MHD_FYZ_PICK(128, true); else MHD_FYZ_PICK(128, false);
   }
 #undef MHD_FYZ_PICK
+  if constexpr (f32) {
+    if (c->opt_tmap && P == 256 && !rag) {      // option tmap: the nine row copies of a stage as tensor-map TMA (UTMALDG)
+      alignas(64) FluidMaps M;
+      int rcm;
+      for (int q = 0; q < 5; ++q) if ((rcm = get_tmap(c, A.u[q], 256, &M.m[q]))) return rcm;
+      if ((rcm = get_tmap(c, A.bd, 256, &M.m[5])) || (rcm = get_tmap(c, A.bo, 256, &M.m[6])) || (rcm = get_tmap(c, A.bx, 256, &M.m[7]))) return rcm;
+      void (*kt)(const YZArgs<real>, const FluidMaps) =
+          want_cmax ? (xt1 ? fluid_yz_ring_tm_kernel<real, T, 256, DR, true, true> : fluid_yz_ring_tm_kernel<real, T, 256, DR, false, true>)
+                    : (xt1 ? fluid_yz_ring_tm_kernel<real, T, 256, DR, true, false> : fluid_yz_ring_tm_kernel<real, T, 256, DR, false, false>);
+      const size_t smem_t = FluidRing<real, 256, true>::smem_bytes(DR);
+      if ((rcm = want_smem(c, (const void*)kt, smem_t))) return rcm;
+      kt<<<grid, 256 / PackOf<T>::L, smem_t, c->stream>>>(A, M);
+      c->launches++;
+      CUDA_TRY(c, cudaGetLastError());
+      swap_fields(c, role, 5);
+      return MHD_OK;
+    }
+  }
   int rc = want_smem(c, (const void*)k, smem);
   if (rc) return rc;
   k<<<grid, P / PackOf<T>::L, smem, c->stream>>>(A);
@@ -1036,6 +1088,7 @@ extern "C" int mhd_set_option(mhd_ctx* c, const char* key, long long value) {
   }
   if (!strcmp(key, "xpack")) { if (value < 1 || value > 3) return fail(c, MHD_EINVAL, "xpack must be 1, 2 or 3"); c->opt_xpack = (int)value; return MHD_OK; }
   if (!strcmp(key, "brows")) { if (value < 1 || value > 2) return fail(c, MHD_EINVAL, "brows must be 1 or 2"); c->opt_brows = (int)value; return MHD_OK; }
+  if (!strcmp(key, "tmap")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "tmap must be 0 or 1"); c->opt_tmap = (int)value; return MHD_OK; }
   if (!strcmp(key, "xfuse")) { if (value < 0 || value > 3) return fail(c, MHD_EINVAL, "xfuse must be 0, 1 (fp32 only), 2 (always) or 3 (fp32, packed)"); c->opt_xfuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "fuse")) { if (value < 0 || value > 2) return fail(c, MHD_EINVAL, "fuse must be 0, 1 or 2"); c->opt_fuse = (int)value; return MHD_OK; }
   if (!strcmp(key, "cmax_reuse")) { if (value < 0 || value > 1) return fail(c, MHD_EINVAL, "cmax_reuse must be 0 or 1"); c->opt_cmax_reuse = (int)value; return MHD_OK; }

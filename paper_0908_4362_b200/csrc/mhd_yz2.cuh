@@ -25,14 +25,17 @@
 #include "mhd_async.cuh"
 #include <type_traits>
 #include "mhd_pack_io.cuh"
+#include <cuda.h>                                         // CUtensorMap (type only; the driver entry point is looked up at run time)
 
 namespace mhd {
 
-template <class real, int TXB>
+// TM: the nine row copies of a stage are tensor-map TMA copies (cp.async.bulk.tensor.3d, SASS UTMALDG), whose shared-memory
+// destination must be 128-byte aligned: the stage is padded to a multiple of 128 bytes
+template <class real, int TXB, bool TM = false>
 struct FluidRing {
   static constexpr int CH = 16 / sizeof(real);            // elements in one 16-byte chunk
   static constexpr int ROW = TXB;
-  static constexpr int STAGE = 9 * ROW + CH;              // u0..u4, bd(q+1), bo(o), bo(o+1), bx, bx chunk at x0+TXB
+  static constexpr int STAGE = 9 * ROW + (TM ? 128 / (int)sizeof(real) : CH);   // u0..u4, bd(q+1), bo(o), bo(o+1), bx, bx chunk at x0+TXB
   static constexpr uint32_t BYTES = STAGE * sizeof(real);
   static size_t smem_bytes(int D) { return (size_t)D * STAGE * sizeof(real) + 2 * D * sizeof(uint64_t); }
 };
@@ -66,9 +69,17 @@ struct FluidRing {
 // consumers keep one running store offset, and the march is unrolled by four with the step number modulo 4 a
 // compile-time constant.
 // RAG: the row ends in a tile narrower than TXB (else the width is a compile-time constant, as the tuned kernel wants)
-template <class real, class T, int TXB, int D, bool XT1, bool CM, bool RAG = false>
-__global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_ring_kernel(const YZArgs<real> A) {
-  using RG = FluidRing<real, TXB>;
+struct FluidMaps { CUtensorMap m[8]; };                  // u0..u4 (sweep roles), B_d, B_o, B_x: 3-D maps (x, y, z), box TXB x 1 x 1
+
+__device__ __forceinline__ void tma_g2s_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(smem_u32(dst)),
+               "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+
+template <class real, class T, int TXB, int D, bool XT1, bool CM, bool RAG, bool TM>
+__device__ __forceinline__ void fluid_yz_ring_body(const YZArgs<real>& A, const CUtensorMap* tm) {
+  using RG = FluidRing<real, TXB, TM>;
   typedef typename PackOf<T>::scalar S;
   constexpr int L = PackOf<T>::L;
   constexpr int NT = TXB / L;                            // threads (all consumers)
@@ -122,6 +133,20 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
       real* st = ring + s * RG::STAGE;
       const uint32_t RB = (uint32_t)w * sizeof(real);
       mbar_expect_tx(&full[s], 9u * RB + 16u);
+      if constexpr (TM) {
+        // coordinates (x, y, z) of the rows (q, o), (q+1, o), (q, o+1): the sweep axis is z when x is t1 (XT1), else y
+        const int qm = map_index1(q, A.nd, A.bc), q1 = map_index1(q + 1, A.nd, A.bc), op = map_index1(o + 1, A.no, A.bc);
+        const int ya = XT1 ? o : qm, za = XT1 ? qm : o;            // row (q, o)
+        const int yb = XT1 ? o : q1, zb = XT1 ? q1 : o;            // row (q+1, o)
+        const int yc = XT1 ? op : qm, zc = XT1 ? qm : op;          // row (q, o+1)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) tma_g2s_3d(st + k * RG::ROW, tm + k, x0, ya, za, &full[s]);
+        tma_g2s_3d(st + 5 * RG::ROW, tm + 5, x0, yb, zb, &full[s]);
+        tma_g2s_3d(st + 6 * RG::ROW, tm + 6, x0, ya, za, &full[s]);
+        tma_g2s_3d(st + 7 * RG::ROW, tm + 6, x0, yc, zc, &full[s]);
+        tma_g2s_3d(st + 8 * RG::ROW, tm + 7, x0, ya, za, &full[s]);
+        bulk_g2s(st + 9 * RG::ROW, b0 + A.src[7] + xc_bytes, 16, &full[s]);
+      } else {
 #pragma unroll
       for (int k = 0; k < 5; ++k) bulk_g2s(st + k * RG::ROW, b0 + A.src[k], RB, &full[s]);
       bulk_g2s(st + 5 * RG::ROW, b1 + A.src[5], RB, &full[s]);               // B_d at the next face
@@ -129,6 +154,7 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
       bulk_g2s(st + 7 * RG::ROW, b0 + A.src[6] + op_bytes, RB, &full[s]);    // B_o at o+1
       bulk_g2s(st + 8 * RG::ROW, b0 + A.src[7], RB, &full[s]);               // B_x
       bulk_g2s(st + 9 * RG::ROW, b0 + A.src[7] + xc_bytes, 16, &full[s]);    // the chunk holding B_x at x0+TXB
+      }
     }
     __syncwarp();
   };
@@ -216,6 +242,16 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_rin
     const unsigned long long cw = warp_max_u64(key_bits(cbest));
     if (lane == 0) publish_max(A.cmax_bits, cw);
   }
+}
+
+template <class real, class T, int TXB, int D, bool XT1, bool CM, bool RAG = false>
+__global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_ring_kernel(const YZArgs<real> A) {
+  fluid_yz_ring_body<real, T, TXB, D, XT1, CM, RAG, false>(A, nullptr);
+}
+// the same with tensor-map copies (option tmap; whole tiles only)
+template <class real, class T, int TXB, int D, bool XT1, bool CM>
+__global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_YZ2_MINB) fluid_yz_ring_tm_kernel(const YZArgs<real> A, const __grid_constant__ FluidMaps M) {
+  fluid_yz_ring_body<real, T, TXB, D, XT1, CM, false, true>(A, M.m);
 }
 
 }  // namespace mhd

@@ -450,6 +450,40 @@ def test_b_pair_two_rows_per_thread(B, shape, bc):
                     assert np.max(np.abs(a - b)) <= 1e-6 * np.max(np.abs(b)), (shape, bc, seg, d, rev)
 
 
+@pytest.mark.parametrize("bc", [P, O])
+def test_fluid_ring_with_tensor_map_copies(B, bc):
+    """option tmap: the nine row copies of a fluid_yz ring stage as tensor-map TMA copies (cp.async.bulk.tensor.3d, SASS
+    UTMALDG) instead of 1-D bulk copies: same bits as the default kernel, and the oracle's values"""
+    nx, ny, nz = 512, 14, 22
+    f0 = random_state(nx, ny, nz, seed=17 + bc)
+    gamma, dt = 5.0 / 3.0, 0.2
+    for seg in (-1, 9):
+        for d in (1, 2):
+            ref = _ref_input(f0, "f32")
+            oracle.fluid(ref, gamma, bc, d, dt)
+            out = []
+            for tmap in (1, 0):
+                s = _solver(B, f0, gamma, bc, "f32", segment=seg, tmap=tmap)
+                s.apply(B.MHD_OP_FLUID, d, 0, dt)
+                out.append(s.get_state())
+                s.close()
+            assert worst(max_rel(out[0], ref)) <= TOL32_STEP, (bc, seg, d)
+            for a, b in zip(out[0], out[1]):
+                assert np.array_equal(a, b), (bc, seg, d)
+    # whole steps with the fused c_max reduction
+    ref = _ref_input(f0, "f32")
+    oracle.step_fixed(ref, gamma, bc, 1, dt)
+    s = _solver(B, f0, gamma, bc, "f32", tmap=1)
+    s.step_index = 1
+    s.step_fixed(1, dt)
+    got = s.get_state()
+    _, cmg = s.cfl_dt(0.8)
+    s.close()
+    assert worst(max_rel(got, ref)) <= TOL32_STEP
+    cm = oracle.cmax([np.array(a, dtype=np.float64) for a in got], gamma, bc)
+    assert abs(cmg - cm) <= 2e-6 * cm
+
+
 @pytest.mark.parametrize("bring", [1])
 @pytest.mark.parametrize("bc", [P, O])
 def test_b_pair_ring_march_fp64(B, bring, bc):
