@@ -57,7 +57,10 @@ size_t mhd_workspace_bytes(int nx, int ny, int nz, int precision);
 /* Create a context for an nx*ny*nz grid (any extents >= 1; an extent of 1 makes that axis
  * degenerate, e.g. 512x1x1 for 1-D runs).  gamma > 1 is the adiabatic index of
  * P = (gamma-1)(E - rho v^2/2 - B^2/2).  No device memory is touched until the first
- * call that needs it (mhd_bind or mhd_set_state).  *out receives the context. */
+ * call that needs it (mhd_bind or mhd_set_state).  *out receives the context.
+ * Every size and both boundary rules give the same results to rounding; the specialised kernels
+ * want nx to be a multiple of 16 bytes (4 floats / 2 doubles), rows of at most 2048 (fp32) / 1024 (fp64) cells and fewer
+ * than 2^31 cells, otherwise slower generic kernels run. */
 int mhd_create(int nx, int ny, int nz, double gamma, int precision, int bc, mhd_ctx** out);
 
 /* Optional.  Use caller-owned DEVICE memory (at least mhd_workspace_bytes, 256-byte aligned) and/or a
