@@ -425,6 +425,26 @@ def main():
             s2.close()
             del s2, ws2, st2
             torch.cuda.empty_cache()
+        # c1 (1-D Brio-Wu 512, fp64, outflow) and c2 (2-D Orszag-Tang 256^2, fp32 and fp64): a few thousand cells, bound by
+        # launch latency (a step is ten launches replayed as a CUDA graph), reported for completeness of "each config"
+        from paper_0908_4362_b200 import inputs as _inp
+        for name, (fgen, shape, p2, ksteps, d2) in {
+                "c1": (_inp.brio_wu, (512, 1, 1), "f64", 100, "configs[0]: 1-D Brio-Wu, 512x1x1, fp64, outflow, cfl 0.8"),
+                "c2_f32": (_inp.orszag_tang, (256, 256, 1), "f32", 500, "configs[1]: 2-D Orszag-Tang, 256x256x1, fp32, periodic, cfl 0.8"),
+                "c2_f64": (_inp.orszag_tang, (256, 256, 1), "f64", 500, "configs[1]: 2-D Orszag-Tang, 256x256x1, fp64, periodic, cfl 0.8")}.items():
+            f2_, m2 = fgen(shape[0])
+            dt2 = np.float32 if p2 == "f32" else np.float64
+            s2 = B.Solver(shape[0], shape[1], shape[2], m2["gamma"], p2, m2["bc"], stream=stream)
+            s2.set_state([np.ascontiguousarray(a, dtype=dt2) for a in f2_])
+            with torch.cuda.stream(stream):
+                s2.step(args.warmup, CFL, sync=True)
+            oms, oclk, _ = timed(s2, stream, ksteps)
+            s2.time()
+            ncell = shape[0] * shape[1] * shape[2]
+            others[name] = {"workload": d2, "dtype": p2, "steps": ksteps, "ms_per_step": oms / ksteps,
+                            "value": ncell * ksteps / (oms * 1e-3), "unit": "cell-updates/s", "clocks": oclk,
+                            "l2": l2_note(8 * ncell * (4 if p2 == "f32" else 8))}
+            s2.close()
 
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
