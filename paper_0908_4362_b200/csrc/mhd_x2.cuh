@@ -138,6 +138,51 @@ __device__ __forceinline__ XRows x_rows(const XArgs<real>& A) {
   return r;
 }
 
+// right_left of the V cells of a thread.  One row per thread in fp32 (T = float, V = 4): the flux evaluation is cell by cell
+// (no stencil), so cells (0,1) and (2,3) run as two f2 packs: FADD2 / FMUL2 / FFMA2 for what was two scalar streams, with
+// the SAME registers (a float4 load puts neighbours in an aligned pair, scalar producers write into their half of a pair), so
+// unlike packing two rows it costs no occupancy.  Results per cell are the same operations in the same order.
+template <class T, int V>
+__device__ __forceinline__ void right_left_cells(const T (&u)[V][5], const BCell<T> (&B)[V], T gamma, T (&R)[V][5], T (&G)[V][5]) {
+#pragma unroll
+  for (int v = 0; v < V; ++v) right_left(u[v], B[v], gamma, R[v], G[v]);
+}
+#ifndef MHD_X2_NO_CELLPACK
+template <>
+__device__ __forceinline__ void right_left_cells<float, 4>(const float (&u)[4][5], const BCell<float> (&B)[4], float gamma,
+                                                           float (&R)[4][5], float (&G)[4][5]) {
+#pragma unroll
+  for (int v = 0; v < 4; v += 2) {
+    f2 uu[5], RR[5], GG[5];
+#pragma unroll
+    for (int c = 0; c < 5; ++c) uu[c] = f2(u[v][c], u[v + 1][c]);
+    BCell<f2> BB;
+    BB.b0 = f2(B[v].b0, B[v + 1].b0); BB.b1 = f2(B[v].b1, B[v + 1].b1); BB.b2 = f2(B[v].b2, B[v + 1].b2);
+    BB.hb2 = f2(B[v].hb2, B[v + 1].hb2);
+    right_left(uu, BB, f2(gamma), RR, GG);
+#pragma unroll
+    for (int c = 0; c < 5; ++c) { R[v][c] = RR[c].v.x; R[v + 1][c] = RR[c].v.y; G[v][c] = GG[c].v.x; G[v + 1][c] = GG[c].v.y; }
+  }
+}
+#endif
+
+// x[v] - d[v] * s for the V cells of a thread (the two update steps of Algorithm 1); fp32 one row per thread: two packs
+template <class T, int V>
+__device__ __forceinline__ void axpy_cells(const T (&d)[V], T s, const T (&x)[V], T (&y)[V]) {
+#pragma unroll
+  for (int v = 0; v < V; ++v) y[v] = fnma_(d[v], s, x[v]);
+}
+#ifndef MHD_X2_NO_CELLPACK
+template <>
+__device__ __forceinline__ void axpy_cells<float, 4>(const float (&d)[4], float s, const float (&x)[4], float (&y)[4]) {
+#pragma unroll
+  for (int v = 0; v < 4; v += 2) {
+    const f2 r = fnma_(f2(d[v], d[v + 1]), f2(s), f2(x[v], x[v + 1]));
+    y[v] = r.v.x; y[v + 1] = r.v.y;
+  }
+}
+#endif
+
 // ---------------------------------------------------------------------------------------------
 // fluid_x of the V cells of one thread, Algorithm 1, in pack arithmetic.
 // sm: 7 groups x 5 components x NT packs.  u[c][v], B[v] in; un[v][c] out.  Contains three barriers;
@@ -149,12 +194,13 @@ __device__ __forceinline__ void fluid_x_core(T* sm, int tid, int tl, int tr, con
   auto S = [&](int group, int comp, int thr) -> T& { return sm[(group * 5 + comp) * NT + thr]; };
   // stage 0: R, G of u^t (Alg. 1 step 4)
   T R[V][5], G[V][5];
+  {
+    T uc[V][5];
 #pragma unroll
-  for (int v = 0; v < V; ++v) {
-    T uu[5];
+    for (int v = 0; v < V; ++v)
 #pragma unroll
-    for (int c = 0; c < 5; ++c) uu[c] = u[c][v];
-    right_left(uu, B[v], gamma, R[v], G[v]);
+      for (int c = 0; c < 5; ++c) uc[v][c] = u[c][v];
+    right_left_cells<T, V>(uc, B, gamma, R, G);
   }
 #pragma unroll
   for (int c = 0; c < 5; ++c) { S(0, c, tid) = R[V - 1][c]; S(1, c, tid) = G[0][c]; }
@@ -168,12 +214,17 @@ __device__ __forceinline__ void fluid_x_core(T* sm, int tid, int tl, int tr, con
 #pragma unroll
     for (int v = 1; v < V; ++v) d1[v] = R[v - 1][c] - G[v][c];
     d1[V] = R[V - 1][c] - S(1, c, tr);
+    {
+      T dd[V], y[V];
 #pragma unroll
-    for (int v = 0; v < V; ++v) uh[v][c] = fnma_(d1[v + 1] - d1[v], qdt, u[c][v]);
+      for (int v = 0; v < V; ++v) dd[v] = d1[v + 1] - d1[v];
+      axpy_cells<T, V>(dd, qdt, u[c], y);
+#pragma unroll
+      for (int v = 0; v < V; ++v) uh[v][c] = y[v];
+    }
   }
   // stage 1: R, G of u^{t+dt/2} (step 7), same B_c
-#pragma unroll
-  for (int v = 0; v < V; ++v) right_left(uh[v], B[v], gamma, R[v], G[v]);
+  right_left_cells<T, V>(uh, B, gamma, R, G);
 #pragma unroll
   for (int c = 0; c < 5; ++c) {
     S(2, c, tid) = R[V - 1][c];      // my last R  -> right neighbour's R[-1]
@@ -206,8 +257,14 @@ __device__ __forceinline__ void fluid_x_core(T* sm, int tid, int tl, int tr, con
 #pragma unroll
   for (int c = 0; c < 5; ++c) {
     phi[0][c] = S(6, c, tl);
+    {
+      T dd[V], y[V];
 #pragma unroll
-    for (int v = 0; v < V; ++v) un[v][c] = fnma_(phi[v + 1][c] - phi[v][c], hdt, u[c][v]);
+      for (int v = 0; v < V; ++v) dd[v] = phi[v + 1][c] - phi[v][c];
+      axpy_cells<T, V>(dd, hdt, u[c], y);
+#pragma unroll
+      for (int v = 0; v < V; ++v) un[v][c] = y[v];
+    }
   }
 }
 
@@ -292,6 +349,14 @@ __device__ __forceinline__ void bpair_x_core(T* sm, int tid, int tl, int tr, con
   for (int p = 0; p < 4; ++p) f[p][0] = S(1, p, tl);
 }
 
+// Alg. 2 step 4 (reading R5) for the V cells of a thread: (ma + mb) / (ra + rb) cell by cell (packing these over cell pairs,
+// like right_left_cells, and likewise the cell-by-cell parts of bpair_x_core, was measured: no gain / 7 % slower)
+template <class T, int V>
+__device__ __forceinline__ void face_velocity(const T (&ma)[V], const T (&mb)[V], const T (&ra)[V], const T (&rb)[V], T (&vt)[V]) {
+#pragma unroll
+  for (int v = 0; v < V; ++v) vt[v] = (ma[v] + mb[v]) * rcp_(ra[v] + rb[v]);
+}
+
 // face velocities and transverse fields of the four flux rows of one thread (Alg. 2 step 4, reading R5:
 // momentum sum over density sum of the two cells sharing the face).  r0, m0: rho, m_x of the thread's own cells.
 template <class real, class T, int V, bool OUT = false>
@@ -301,17 +366,13 @@ __device__ __forceinline__ void bpair_x_inputs(const XArgs<real>& A, const XRows
   auto ld = [&](const real* f, int oa, int ob, T (&v)[V]) { xload(f, oa, ob, v, A.one); };
   ld(A.u[0], q.o[1], q.o[2], r0); ld(A.u[1], q.o[1], q.o[2], m0);
   ld(A.u[0], q.o[0], q.o[1], r); ld(A.u[1], q.o[0], q.o[1], m);                  // rows j-1 (, j)
-#pragma unroll
-  for (int v = 0; v < V; ++v) vt[0][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
+  face_velocity<T, V>(m, m0, r, r0, vt[0]);
   ld(A.u[0], q.o[2], q.o[3], r); ld(A.u[1], q.o[2], q.o[3], m);                  // rows j+1 (, j+2)
-#pragma unroll
-  for (int v = 0; v < V; ++v) vt[1][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
+  face_velocity<T, V>(m0, m, r0, r, vt[1]);
   ld(A.u[0], q.okm[0], q.okm[1], r); ld(A.u[1], q.okm[0], q.okm[1], m);
-#pragma unroll
-  for (int v = 0; v < V; ++v) vt[2][v] = (m[v] + m0[v]) * rcp_(r[v] + r0[v]);
+  face_velocity<T, V>(m, m0, r, r0, vt[2]);
   ld(A.u[0], q.okp[0], q.okp[1], r); ld(A.u[1], q.okp[0], q.okp[1], m);
-#pragma unroll
-  for (int v = 0; v < V; ++v) vt[3][v] = (m0[v] + m[v]) * rcp_(r0[v] + r[v]);
+  face_velocity<T, V>(m0, m, r0, r, vt[3]);
   ld(A.by, q.o[1], q.o[2], b[0]);
   ld(A.by, q.o[2], q.o[3], b[1]);
   ld(A.bz, q.o[1], q.o[2], b[2]);
@@ -332,6 +393,21 @@ __device__ __forceinline__ void x_centre(const T (&bxe)[V + 1], const T (&bya)[V
   for (int v = 0; v < V; ++v)
     B[v].set(half * (bxe[v] + bxe[v + 1]), half * (bya[v] + byb[v]), half * (bza[v] + bzb[v]));
 }
+#ifndef MHD_X2_NO_CELLPACK
+template <>
+__device__ __forceinline__ void x_centre<float, 4>(const float (&bxe)[5], const float (&bya)[4], const float (&byb)[4], const float (&bza)[4],
+                                                   const float (&bzb)[4], BCell<float> (&B)[4]) {
+  const f2 half(0.5f);
+#pragma unroll
+  for (int v = 0; v < 4; v += 2) {           // cells (v, v+1) as one pack (see right_left_cells)
+    BCell<f2> BB;
+    BB.set(half * (f2(bxe[v], bxe[v + 1]) + f2(bxe[v + 1], bxe[v + 2])), half * (f2(bya[v], bya[v + 1]) + f2(byb[v], byb[v + 1])),
+           half * (f2(bza[v], bza[v + 1]) + f2(bzb[v], bzb[v + 1])));
+    B[v].b0 = BB.b0.v.x; B[v + 1].b0 = BB.b0.v.y; B[v].b1 = BB.b1.v.x; B[v + 1].b1 = BB.b1.v.y;
+    B[v].b2 = BB.b2.v.x; B[v + 1].b2 = BB.b2.v.y; B[v].hb2 = BB.hb2.v.x; B[v + 1].hb2 = BB.hb2.v.y;
+  }
+}
+#endif
 
 template <class real, class T, int V>
 __device__ __forceinline__ void x_store_u_and_cmax(const XArgs<real>& A, const XRows& q, const T (&un)[V][5],
