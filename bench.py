@@ -428,10 +428,15 @@ def main():
         # c1 (1-D Brio-Wu 512, fp64, outflow) and c2 (2-D Orszag-Tang 256^2, fp32 and fp64): a few thousand cells, bound by
         # launch latency (a step is ten launches replayed as a CUDA graph), reported for completeness of "each config"
         from paper_0908_4362_b200 import inputs as _inp
-        for name, (fgen, shape, p2, ksteps, d2) in {
-                "c1": (_inp.brio_wu, (512, 1, 1), "f64", 100, "configs[0]: 1-D Brio-Wu, 512x1x1, fp64, outflow, cfl 0.8"),
-                "c2_f32": (_inp.orszag_tang, (256, 256, 1), "f32", 500, "configs[1]: 2-D Orszag-Tang, 256x256x1, fp32, periodic, cfl 0.8"),
-                "c2_f64": (_inp.orszag_tang, (256, 256, 1), "f64", 500, "configs[1]: 2-D Orszag-Tang, 256x256x1, fp64, periodic, cfl 0.8")}.items():
+        # ... and the largest sizes of the paper's own Tables 1 and 2 with the paper's GTX 480 ms per step beside them
+        # (another machine: context)
+        for name, (fgen, shape, p2, ksteps, d2, paper_ms) in {
+                "c1": (_inp.brio_wu, (512, 1, 1), "f64", 100, "configs[0]: 1-D Brio-Wu, 512x1x1, fp64, outflow, cfl 0.8", 3.21),
+                "c2_f32": (_inp.orszag_tang, (256, 256, 1), "f32", 500, "configs[1]: 2-D Orszag-Tang, 256x256x1, fp32, periodic, cfl 0.8", 12.48),
+                "c2_f64": (_inp.orszag_tang, (256, 256, 1), "f64", 500, "configs[1]: 2-D Orszag-Tang, 256x256x1, fp64, periodic, cfl 0.8", 21.59),
+                "t1_4096_f32": (_inp.brio_wu, (4096, 1, 1), "f32", 200, "paper Table 1: 1-D Brio-Wu, 4096x1x1, fp32", 4.31),
+                "t2_1024_f32": (_inp.orszag_tang, (1024, 1024, 1), "f32", 200, "paper Table 2: 2-D Orszag-Tang, 1024x1024x1, fp32", 96.43),
+                "t2_1024_f64": (_inp.orszag_tang, (1024, 1024, 1), "f64", 200, "paper Table 2: 2-D Orszag-Tang, 1024x1024x1, fp64", 144.48)}.items():
             f2_, m2 = fgen(shape[0])
             dt2 = np.float32 if p2 == "f32" else np.float64
             s2 = B.Solver(shape[0], shape[1], shape[2], m2["gamma"], p2, m2["bc"], stream=stream)
@@ -443,7 +448,8 @@ def main():
             ncell = shape[0] * shape[1] * shape[2]
             others[name] = {"workload": d2, "dtype": p2, "steps": ksteps, "ms_per_step": oms / ksteps,
                             "value": ncell * ksteps / (oms * 1e-3), "unit": "cell-updates/s", "clocks": oclk,
-                            "l2": l2_note(8 * ncell * (4 if p2 == "f32" else 8))}
+                            "l2": l2_note(8 * ncell * (4 if p2 == "f32" else 8)),
+                            "paper_gtx480_ms_per_step": paper_ms, "vs_paper_gtx480": paper_ms / (oms / ksteps)}
             s2.close()
 
     cpu = None
