@@ -379,6 +379,46 @@ def test_badvect_constant_velocity_linear_data_exact(d, t, v):
 
 
 # ---------------------------------------------------------------------------------------------
+# P10b: along an axis of extent 1 Algorithm 2 collapses (reading R10): B_t comes back bit for bit and B_d changes by the
+# difference of the first-order edge fluxes f = (vt B_t) dt of the rows tau+1 and tau.  Hand-derivable from
+# eqs (20)-(22): every index along d maps to the only cell, so vg = vt, both upwind candidates coincide and the limited
+# differences vanish.  (The CUDA path has a closed-form kernel for this case; this pins the oracle's side of it.)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [P, O])
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_badvect_along_an_extent_one_axis_is_the_constraint_term_alone(d, bc):
+    rng = np.random.default_rng(5 + d)
+    n = [6, 5, 7]
+    n[d] = 1
+    shape = (n[2], n[1], n[0])
+    f = c64([1.0 + 0.3 * rng.random(shape)] + [rng.standard_normal(shape) * 0.4 for _ in range(3)] + [10.0 + rng.random(shape)] +
+            [rng.standard_normal(shape) * 0.5 for _ in range(3)])
+    dt = 0.37
+    for t in ((d + 1) % 3, (d + 2) % 3):
+        g = [a.copy() for a in f]
+        oracle.badvect(g, 5.0 / 3.0, bc, d, t, dt)
+        ax = 2 - t                                           # numpy axis of direction t
+        def shift(a, k):                                     # a[tau + k] with the boundary rule
+            if bc == P:
+                return np.roll(a, -k, axis=ax)
+            idx = np.clip(np.arange(a.shape[ax]) + k, 0, a.shape[ax] - 1)
+            return np.take(a, idx, axis=ax)
+        rho, md, bt = f[0], f[1 + d], f[5 + t]
+        flux = lambda k: (((shift(md, k - 1) + shift(md, k)) / (shift(rho, k - 1) + shift(rho, k))) * shift(bt, k)) * dt
+        # row tau+1 uses the MAPPED cells tau and tau+1 (at a clamped last row both are the last cell)
+        f_here = flux(0)
+        if bc == P:
+            f_next = flux(1)
+        else:
+            f_next = (((md + shift(md, 1)) / (rho + shift(rho, 1))) * shift(bt, 1)) * dt
+        assert np.array_equal(g[5 + t], f[5 + t])            # advected into itself, bit for bit
+        want = f[5 + d] + (f_next - f_here)
+        assert np.abs(g[5 + d] - want).max() <= 4e-16 * max(1.0, np.abs(want).max())
+        for k in range(5):
+            assert np.array_equal(g[k], f[k])
+
+
+# ---------------------------------------------------------------------------------------------
 # P11: brute force on tiny grids against the independently structured NumPy restatement
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("shape", [(4, 1, 1), (1, 5, 1), (1, 1, 4), (4, 4, 1), (4, 3, 2), (7, 5, 6), (2, 2, 2)])
