@@ -157,6 +157,7 @@ static int carve(mhd_ctx* c) {
   }
   c->sc = (Scalars*)(base + 16 * c->field_bytes);
   c->diag = (double*)(base + 16 * c->field_bytes + 256);
+  c->n_tmap = 0;                       // tensor maps are keyed by buffer address: a new workspace invalidates them
   CUDA_TRY(c, cudaMemsetAsync(c->sc, 0, kScalarBlock, c->stream));
   return MHD_OK;
 }
