@@ -183,6 +183,36 @@ int mhd_viz_volume(mhd_ctx* ctx, int field, double vmin, double vmax, const unsi
  * Unknown keys and out-of-range values return MHD_EINVAL. */
 int mhd_set_option(mhd_ctx* ctx, const char* key, long long value);
 
+/* c_max of eq (18) WITHOUT a context and WITHOUT any allocation, for callers that cannot call
+ * cudaMalloc: code that lives inside a host program which owns all device memory through its own pool and forbids
+ * allocations behind its back, loops that cannot afford cudaMalloc's device-wide synchronisation, processes already at
+ * their memory limit.  (Every other compute call needs a context, whose workspace is cudaMalloc'ed by the library or by
+ * whoever passes it to mhd_bind.)  The call issues no cudaMalloc / cudaFree / cudaMallocAsync, creates no stream or event
+ * and makes no host allocation of its own: it enqueues one 256-byte memset and one kernel on `cuda_stream` and returns.
+ *   fields_device[0..7]  DEVICE pointers, same order, layout and precision rules as mhd_set_state; only read
+ *   nx, ny, nz, gamma, precision, bc   as in mhd_create
+ *   cuda_stream          a cudaStream_t passed as void* (NULL = the default stream)
+ *   cmax_device          DEVICE pointer to one double: receives c_max (fp32 states: the float maximum, widened).
+ *                        Written as the reduction produced it: there is no counterpart of mhd_cfl_dt's
+ *                        MHD_ENONFINITE here, so test it for finite and > 0 before forming dt = cfl / c_max.
+ *   errbuf, errbuf_len   optional HOST buffer for the message of a failure (may be NULL / 0)
+ * Does not synchronise: the result is there once work enqueued on `cuda_stream` up to this call has finished.
+ * The kernel's scratch (per-block partial maxima and a block counter) is a fixed 262400-byte array inside the library
+ * image; every GPU on which libmhd.so's kernels are loaded holds it until the process exits.  Consequences:
+ *   - LIMIT: nx*ny*nz <= 2^27 = 134217728 cells (512^3).  Larger grids are refused with MHD_EINVAL and a message;
+ *     nothing is launched.
+ *   - All calls on one GPU share that array, from any thread, stream or context.  Two calls whose kernels can be in
+ *     flight at the same time on one GPU race on it and both results are garbage: keep such calls on one stream, or
+ *     order them yourself.  Calls on different GPUs are independent.
+ *   - The FIRST call on each device (with that device current) also looks up the array's device address
+ *     (cudaGetSymbolAddress, which loads the library's kernels onto the device if nothing has yet).  Make that first
+ *     call during start-up, outside any stream capture.
+ * The result equals mhd_cfl_dt's c_max of a context holding the same state (same per-cell arithmetic; a maximum does
+ * not depend on the order it is taken in).  MHD_EINVAL: NULL pointer, extent < 1, gamma <= 1, unknown enum, too many
+ * cells; MHD_ECUDA: a CUDA call failed. */
+int mhd_cmax_noalloc(const void* const fields_device[8], int nx, int ny, int nz, double gamma, int precision, int bc,
+                     void* cuda_stream, double* cmax_device, char* errbuf, size_t errbuf_len);
+
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches claim). */
 long long mhd_launch_count(const mhd_ctx* ctx);
 

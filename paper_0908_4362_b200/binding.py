@@ -55,6 +55,7 @@ SIGNATURES = {
     "mhd_viz_slice": (c_int, [c_void_p, c_int, c_int, c_double, c_double, c_void_p, c_void_p]),
     "mhd_viz_volume": (c_int, [c_void_p, c_int, c_double, c_double, c_void_p, c_double, c_void_p]),
     "mhd_set_option": (c_int, [c_void_p, c_char_p, c_longlong]),
+    "mhd_cmax_noalloc": (c_int, [_P8, c_int, c_int, c_int, c_double, c_int, c_int, c_void_p, c_void_p, c_char_p, c_size_t]),
     "mhd_launch_count": (c_longlong, [c_void_p]),
     "mhd_last_error": (c_char_p, [c_void_p]),
     "mhd_version": (c_char_p, []),
@@ -84,6 +85,7 @@ mhd_set_step_index = _lib.mhd_set_step_index
 mhd_get_time = _lib.mhd_get_time
 mhd_diagnostics = _lib.mhd_diagnostics
 mhd_set_option = _lib.mhd_set_option
+mhd_cmax_noalloc = _lib.mhd_cmax_noalloc
 mhd_launch_count = _lib.mhd_launch_count
 mhd_last_error = _lib.mhd_last_error
 mhd_version = _lib.mhd_version

@@ -16,7 +16,7 @@ LIB = os.path.join(HERE, "libmhd.so")
 # the same sources with -DMHD_JITTER (csrc/mhd_async.cuh): random sleeps around every mbarrier operation, for
 # tests/test_gpu_jitter.py (compute-sanitizer is closed on this pool); never loaded by the product path
 LIB_JITTER = os.path.join(HERE, "libmhd_jitter.so")
-SOURCES = ["mhd_api.cu"]
+SOURCES = ["mhd_api.cu", "mhd_noalloc.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-shared", "-Xcompiler", "-fPIC", "--cudart=static",
