@@ -37,14 +37,23 @@ def worst(d):
 # fp32 evaluation order -- the oracle's own included -- lands up to ~1e-3 from the fp64 result in a few dozen cells.
 # At those cells "the" fp32 answer does not exist, so the yardstick is the oracle's own sensitivity on the same block:
 # oracle<float>, and oracle<double> from inputs perturbed by +-6e-8 relative (half an fp32 ulp), TIE_WITNESSES times.
-# A block passes when it meets the plain 1e-5, or when
-#   max error        <= 1e-5 + 1.5 x (largest deviation any witness shows from oracle<double>),
+# A block passes when it meets the plain 1e-5 everywhere, or when
+#   every cell above 1e-5 lies within TIE_RADIUS cells (per axis) of a cell where some WITNESS is above 1e-5 too -- the
+#     excuse is by LOCATION: a cell the witnesses do not point at must meet the plain 1e-5, so a seam, halo or
+#     ghost-thread bug of a few dozen cells by 1e-3 somewhere else in a blast-wave block fails (count printed, must be 0),
+#   max error        <= 1e-5 + 1.5 x (largest deviation any witness shows from oracle<double>), and <= TIE_CEILING,
 #   cells above 1e-5 <= 2 x (largest such count among the witnesses) + 16,
 #   mean error       <= 1e-6
 # (measured on c3, 256^3, 6 steps: ratio of maxima <= 1.32, ratio of counts <= 1.76, mean <= 5e-7; an IEEE-division,
 # no-FMA build of the kernels gives the same figures, so none of it is MUFU or contraction).
+# Why a radius: a tie flips the flux of ONE edge; which of the 1 + TIE_WITNESSES evaluations flips at a given edge is
+# a coin toss per edge, and the cells that see the flip are that edge's two cells and, through the operators that
+# follow in the same step, their neighbours at a much smaller amplitude (tests/test_parity_gate.py: an fp32 evaluation
+# that is none of the witnesses is covered at radius 3 by two witnesses already, and at radius 2 never).
 # ---------------------------------------------------------------------------------------------------------------
 TIE_WITNESSES = 8
+TIE_RADIUS = 3
+TIE_CEILING = 5e-3
 
 
 def fp32_step_gate(got, before, gamma, bc, k, dt, core=None, scale=None, tol=1e-5, tag=""):
@@ -57,7 +66,7 @@ def fp32_step_gate(got, before, gamma, bc, k, dt, core=None, scale=None, tol=1e-
     got = [np.asarray(a, dtype=np.float64) for a in got]
     if scale is None:
         scale = {g: max(float(np.abs(ref[i]).max()) for i in idx) for g, idx in GROUPS.items()}
-    out, wit = {}, None
+    out, wit, hot = {}, None, None
     for g, idx in GROUPS.items():
         e = np.stack([np.abs(got[i][core] - ref[i][core]) for i in idx]) / scale[g]
         out[g] = float(e.max())
@@ -76,9 +85,25 @@ def fp32_step_gate(got, before, gamma, bc, k, dt, core=None, scale=None, tol=1e-
         wmax = max(float(w.max()) for w in ws)
         wcount = max(int((w > tol).sum()) for w in ws)
         n_bad = int((e > tol).sum())
+        # where the witnesses are sensitive, on the WHOLE block (a tie just outside the core reaches into it), in ANY of
+        # the eight fields (the flipped edge flux of B reaches m and E through the fluid operators that follow in the
+        # same step, at a hundredth of the amplitude), widened by TIE_RADIUS cells per axis
+        if hot is None:
+            hot = np.zeros(ref[0].shape, dtype=bool)
+            for w in wit:
+                for g2, idx2 in GROUPS.items():
+                    for i in idx2:
+                        hot |= np.abs(w[i] - ref[i]) > tol * scale[g2]
+        from scipy import ndimage
+        unexcused = {}
+        for r in range(TIE_RADIUS + 2):
+            near = hot if r == 0 else ndimage.binary_dilation(hot, structure=np.ones((3, 3, 3), bool), iterations=r)
+            unexcused[r] = int(((e > tol).any(axis=0) & ~near[core]).sum())
         print(f"fp32 tie gate {tag} step {k} {g}: max {out[g]:.2e} in {n_bad} cells; witnesses max {wmax:.2e} in <= {wcount} cells; "
-              f"vs oracle<float> {float(np.stack([np.abs(got[i][core] - wit[0][i][core]) for i in idx]).max()) / scale[g]:.2e}")
-        assert out[g] <= tol + 1.5 * wmax, (tag, k, g, out[g], wmax)
+              f"vs oracle<float> {float(np.stack([np.abs(got[i][core] - wit[0][i][core]) for i in idx]).max()) / scale[g]:.2e}; "
+              f"cells above tol farther than r from every witness-sensitive cell, r: count = {unexcused}")
+        assert unexcused[TIE_RADIUS] == 0, (tag, k, g, unexcused)
+        assert out[g] <= tol + 1.5 * wmax and out[g] <= TIE_CEILING, (tag, k, g, out[g], wmax)
         assert n_bad <= 2 * wcount + 16, (tag, k, g, n_bad, wcount)
         assert float(e.mean()) <= 1e-6, (tag, k, g, float(e.mean()))
     return out
