@@ -171,7 +171,8 @@ int mhd_viz_volume(mhd_ctx* ctx, int field, double vmin, double vmax, const unsi
  *             pairs only.  Measured slower than the two-kernel path on B200, hence not the default.
  *   "cmax_reuse" 1 (default) mhd_cfl_dt returns the cached c_max while the state is unchanged | 0 always reduces
  *   "path"    0 auto (default) | 1 generic marching kernels only (any extents, both BCs)
- *   "segment" cells per block along the sweep for the marching kernels (-1 auto, 0 = whole pencil)
+ *   "segment" cells per block along the sweep for the marching kernels (-1 auto, 0 = whole pencil); the fused sweeps
+ *             of "fuse" 1 / 2 raise a value below 16 to 16 (or to the whole pencil where that is shorter)
  *   "block"   threads per block of the generic kernels (multiple of 32 in [32, 256])
  *   "brows"   B pair along y, z in fp32 on 256-column tiles: 2 (default) two rows per thread where the extent along the other
  *             transverse axis is even | 1 one row per thread

@@ -1,6 +1,6 @@
 """Build libmhd.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_0908_4362_b200.build [--force] [--verbose]
+    python -m paper_0908_4362_b200.build [--force] [--verbose] [--jitter]
 
 The shared library is git-ignored but travels to the GPU box with the repo snapshot.
 """
@@ -41,20 +41,27 @@ def _compile(lib: str, extra, verbose: bool) -> None:
         raise RuntimeError(f"nvcc failed building {os.path.basename(lib)}")
 
 
+def _stale(lib: str, force: bool) -> bool:
+    return force or not os.path.exists(lib) or os.path.getmtime(lib) < _newest_source_mtime()
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    newest = _newest_source_mtime()
-    jobs = [(lib, extra) for lib, extra in ((LIB, []), (LIB_JITTER, ["-DMHD_JITTER"]))
-            if force or not os.path.exists(lib) or os.path.getmtime(lib) < newest]
-    if len(jobs) == 2 and not verbose:             # both stale: compile them side by side
-        import concurrent.futures
-        with concurrent.futures.ThreadPoolExecutor(2) as ex:
-            for f in [ex.submit(_compile, lib, extra, False) for lib, extra in jobs]:
-                f.result()
-    else:
-        for lib, extra in jobs:
-            _compile(lib, extra, verbose)
+    """The product library only.  (The jitter build is test infrastructure: build_jitter(), called by the test that
+    loads it, so that importing the package never waits for, or fails on, a second nvcc run.)"""
+    if _stale(LIB, force):
+        _compile(LIB, [], verbose)
     return LIB
 
 
+def build_jitter(force: bool = False, verbose: bool = False) -> str:
+    """libmhd_jitter.so for tests/test_gpu_jitter.py; never loaded by the product path."""
+    if _stale(LIB_JITTER, force):
+        _compile(LIB_JITTER, ["-DMHD_JITTER"], verbose)
+    return LIB_JITTER
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--jitter" in sys.argv:
+        print(build_jitter(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

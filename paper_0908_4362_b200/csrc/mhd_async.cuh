@@ -66,7 +66,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // One lane of a fully converged warp.  ptxas recognises the elect.sync predicate: a cp.async.bulk guarded by it
 // becomes one UBLKCP with operands in uniform registers.  Guarded by a lane-index test instead, every copy is
 // wrapped in an ELECT / 5 x R2UR.BROADCAST / BRA.U.ANY loop over the active lanes (10 instructions per copy,
-// measured: 12 % of the B-pair ring kernel's issued instructions, profiles/r01_c4_step_ncu_full_c.md).
+// measured: 12 % of the B-pair ring kernel's issued instructions, a round-1 ncu capture; today's opcode mix is in profiles/r02_c4_step_ncu_full.md).
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile(

@@ -89,25 +89,15 @@ __global__ void __launch_bounds__(TXB / PackOf<T>::L, MHD_BRING_MINB) bpair_ring
   // warp-uniform (block indices, kernel parameters, the march step), so they are straight-line UBLKCPs (mhd_async.cuh).
   // Sources are  rho + (march offset) + (row / chunk byte offset of this block) + A.src[field]  (A.src in the constant bank)
   constexpr long long ES = (long long)sizeof(real);
-#ifdef MHD_EXP_L2FEED
-  const long long om_b = (long long)(((o - 1) & 7) * A.so + x0) * ES, o_b = (long long)((o & 7) * A.so + x0) * ES, op_b = (long long)(((o + 1) & 7) * A.so + x0) * ES;
-#else
   const long long om_b = (long long)(map_index1(o - 1, A.no, A.bc) * A.so + x0) * ES, o_b = (long long)(o * A.so + x0) * ES,
                   op_b = (long long)(map_index1(o + 1, A.no, A.bc) * A.so + x0) * ES;
-#endif
   const long long cl_b = o_b + (long long)((xl / CH) * CH - x0) * ES, cr_b = o_b + (long long)((xr / CH) * CH - x0) * ES;   // the 16-byte chunks holding columns x0-1, x0+TXB of row o
   auto produce = [&](int itp) {                           // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
     if (elect_one()) {
-#ifdef MHD_EXP_L2FEED
-      // experiment: every block reads the same few rows, so the inputs come out of L2 (results are wrong on purpose)
-      const int od = (map_index1(n0 - 4 + itp, A.nd, A.bc) & 15) * A.sd;
-      const int odl = (map_index1(n0 - 8 + itp, A.nd, A.bc) & 15) * A.sd;
-#else
       const int od = map_index1(n0 - 4 + itp, A.nd, A.bc) * A.sd;
       const int odl = map_index1(n0 - 8 + itp, A.nd, A.bc) * A.sd;        // B_d of the cell finished at this step
-#endif
       real* st = ring + s * RG::STAGE;
       uint64_t* bar = &full[s];
       const uint32_t RB = (uint32_t)w * sizeof(real);

@@ -5,8 +5,9 @@
 //
 // Arithmetic policy: the step is close to the ALU/issue roofline, so the
 // special functions are the cheap ones.  fp32: MUFU.RCP / MUFU.SQRT (rcp.approx.ftz, sqrt.approx.ftz,
-// <= 1-2 ulp, no slow path) -- far inside the 1e-5 per-step tolerance.  fp64: IEEE division and sqrt
-// (1e-12 tolerance).  No --use_fast_math: the discrete switches (a*b > 0, vh > 0) see IEEE products.
+// <= 1-2 ulp, no slow path) -- far inside the 1e-5 per-step tolerance.  fp64: MUFU.RCP64H / MUFU.RSQ64H seed plus one
+// third-order correction (rcp_, sqrt_ below: an ulp or two, no slow path; the 1e-12 tolerance leaves 10^4).
+// No --use_fast_math: the discrete switches (a*b > 0, vh > 0) see IEEE products.
 #pragma once
 #include <cuda_runtime.h>
 #include "mhd_pack.cuh"
@@ -43,7 +44,7 @@ __device__ __forceinline__ float rcp_(float x) { return __fdiv_rn(1.0f, x); }
 // fp64: MUFU.RCP64H seed (relative error e <= 2^-23) + ONE third-order step  r (1 + e + e^2),  e = 1 - x r:  error e^3
 // = 2^-69, three dependent DFMAs, no slow path and no range check (IEEE division: ~10 DFMAs plus a slow path; two
 // Newton steps: four).  The fp64 kernels are bound by the FP64 pipe and by the latency of exactly these chains
-// (profiles/r01_c5_step_ncu_full_d.md).  x = 0 or denormal gives NaN, which only ever reaches a discarded select
+// (profiles/r02_c5_step_ncu_full.md).  x = 0 or denormal gives NaN, which only ever reaches a discarded select
 // operand (vl_full with a*b <= 0).
 __device__ __forceinline__ double rcp_(double x) {
   double r;

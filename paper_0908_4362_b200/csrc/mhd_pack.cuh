@@ -2,7 +2,7 @@
 // instructions of sm_100a (PTX add/mul/fma.rn.f32x2 -> SASS FADD2 / FMUL2 / FFMA2).
 //
 // Why: the fp32 sweep kernels are bound by instruction issue, not by HBM or by the FMA pipe
-// (profiles/r01_c4_step_ncu_full.md: ~165 of ~280 issued instructions per cell are FADD/FMUL/FFMA).
+// (round-1 ncu capture of the scalar kernels: ~165 of ~280 issued instructions per cell are FADD/FMUL/FFMA).
 // A packed instruction occupies the FMA pipe for two cycles but only ONE issue slot
 // (measured on B200 with a throw-away issue-rate loop: FFMA 3.83 warp-inst/clk/SM, FFMA2 1.97), so
 // a thread that advances two adjacent pencils in f2 arithmetic issues half the floating-point

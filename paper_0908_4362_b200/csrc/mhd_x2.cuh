@@ -8,7 +8,7 @@
 //
 //  * T = f2 (mhd_pack.cuh): a thread owns the same V columns of TWO adjacent rows (j, j+1) and advances
 //    both with packed fp32 instructions (FADD2/FMUL2/FFMA2): the scalar x kernels are issue-bound
-//    (profiles/r01_c4_step_ncu_full_b.md: 273 and 194 issued instructions per cell, 65-68 % issue
+//    (round-1 ncu capture: 273 and 194 issued instructions per cell, 65-68 % issue
 //    utilisation), and about 60 % of what they issue is FADD/FMUL/FFMA.  The shared-memory exchange moves
 //    8-byte packs (LDS.64/STS.64), so those instructions halve per cell as well.
 //  * the reverse operator needs no second pass over the state: in a reverse sweep the B pair runs BEFORE

@@ -107,27 +107,21 @@ __device__ __forceinline__ void fluid_yz_ring_body(const YZArgs<real>& A, const 
 
   // ---- producer duty: one elected lane of the warp on duty issues the 10 copies of a stage; every operand is
   // warp-uniform (block indices, kernel parameters, the march step), so the copies are straight-line UBLKCPs ------
-#ifdef MHD_EXP_L2FEED
-  const int rowbase = x0 + (o & 7) * A.so;       // experiment: inputs out of L2 (results are wrong on purpose)
-#else
   const int rowbase = x0 + o * A.so;
-#endif
   const long long op_bytes = (long long)((map_index1(o + 1, A.no, A.bc) - o) * A.so) * (long long)sizeof(real);
   const long long xc_bytes = (long long)((map_index1(x0 + w, A.nx, A.bc) / RG::CH) * RG::CH - x0) * (long long)sizeof(real);   // B_x at x0+w lives in this 16-byte chunk
   auto produce = [&](int itp) {                          // called by one whole, converged warp
     const unsigned s = (unsigned)itp % D;
-#ifndef MHD_BUG_NO_EMPTY_WAIT        // (fault injection for tests/test_gpu_jitter.py: refill a stage without waiting for its readers)
+#if defined(MHD_BUG_NO_EMPTY_WAIT) && !defined(MHD_JITTER)
+#error "MHD_BUG_NO_EMPTY_WAIT injects a race on purpose: only the jitter build (-DMHD_JITTER, libmhd_jitter.so) may define it"
+#endif
+#ifndef MHD_BUG_NO_EMPTY_WAIT        // (fault injection, jitter build only: refill a stage without waiting for its readers)
     if (itp >= D) mbar_wait(&empty[s], (((unsigned)itp / D) & 1) ^ 1);
 #endif
     if (elect_one()) {
       const int q = n0 - 3 + itp;
-#ifdef MHD_EXP_L2FEED
-      const int od = (map_index1(q, A.nd, A.bc) & 15) * A.sd;
-      const int od1 = (map_index1(q + 1, A.nd, A.bc) & 15) * A.sd;
-#else
       const int od = map_index1(q, A.nd, A.bc) * A.sd;
       const int od1 = map_index1(q + 1, A.nd, A.bc) * A.sd;
-#endif
       const char* b0 = reinterpret_cast<const char*>(A.u[0] + od + rowbase);     // row (q, o), columns x0.. of field u[0]
       const char* b1 = reinterpret_cast<const char*>(A.u[0] + od1 + rowbase);    // row (q+1, o)
       real* st = ring + s * RG::STAGE;

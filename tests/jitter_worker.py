@@ -14,7 +14,11 @@ import numpy as np
 CASES = [((256, 24, 40), "f32", {}), ((256, 24, 40), "f64", {}), ((128, 40, 33), "f32", {"segment": 12}),
          ((128, 40, 36), "f32", {"fuse": 1}), ((128, 36, 40), "f64", {"fuse": 1}), ((256, 40, 36), "f32", {"fuse": 2}),
          ((64, 40, 36), "f64", {"fuse": 1, "segment": 16}), ((512, 16, 12), "f32", {}),
-         ((256, 24, 40), "f32", {"brows": 1})]          # the one-row fp32 B pair (default: two rows per thread)
+         ((256, 24, 40), "f32", {"brows": 1}),          # the one-row fp32 B pair (default: two rows per thread)
+         # ring plumbing added in round 2: a narrower last tile per row (nx = 320, 200, 72: run-time expect_tx byte counts,
+         # moved right-chunk slots), outflow boundaries on the ring kernels ("bc": 1), the tensor-map producer (tmap = 1)
+         ((320, 24, 40), "f32", {}), ((200, 24, 20), "f32", {"bc": 1}), ((72, 20, 24), "f64", {}),
+         ((512, 16, 24), "f32", {"tmap": 1}), ((320, 20, 24), "f64", {"bc": 1})]
 
 
 def run_all():
@@ -24,7 +28,8 @@ def run_all():
     for i, (shape, prec, opts) in enumerate(CASES):
         nx, ny, nz = shape
         f = [np.ascontiguousarray(a, dtype=np.float32 if prec == "f32" else np.float64) for a in random_state(nx, ny, nz, seed=40 + i)]
-        s = B.Solver(nx, ny, nz, 1.4, prec, 0)
+        opts = dict(opts)
+        s = B.Solver(nx, ny, nz, 1.4, prec, opts.pop("bc", 0))
         s.set_option("graph", 0)
         for k, v in opts.items():
             s.set_option(k, v)

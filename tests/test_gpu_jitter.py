@@ -22,6 +22,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def test_jittered_build_gives_identical_bits(tmp_path):
     from paper_0908_4362_b200 import build as bld
     bld.build()
+    bld.build_jitter()         # nvcc runs on the GPU box only if the library did not travel with the snapshot
     assert os.path.exists(bld.LIB_JITTER)
     from tests import jitter_worker
     ref = jitter_worker.run_all()
