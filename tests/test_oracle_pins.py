@@ -660,3 +660,64 @@ def test_viz_slice_is_a_table_lookup_and_volume_follows_the_compositing_closed_f
     lut3 = lut.copy(); lut3[:, 3] = 255
     front = viz.volume_rgba(f, 0, g, 0, lo, hi, lut3, 1.0)
     assert np.array_equal(front[..., :3], viz.slice_rgba(f, 0, g, 0, 0, lo, hi, lut3)[..., :3]) and np.all(front[..., 3] == 255)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# The one discontinuous decision of the scheme: the upwind switch of eq (21), PAPER.md:152 --
+#     (v B)_{i+1/2} = (v B)_i  if  v_{i+1/2} > 0,     (v B)_{i+1}  if  v_{i+1/2} <= 0
+# so at an EXACT tie v_{i+1/2} = 0 the flux comes from cell i+1.  Random data never hit the tie; mirror-symmetric data
+# (the blast waves c3, E4, E6) do.  Worked example, every number dyadic until the one limiter quotient:
+#   16 cells along d, periodic, rho = 1, B_t = 1, dt = 1/2, velocity along d
+#     v  = 0 0 0 0 | 1 1 1 1 | -1 -1 -1 -1 | 0 0 0 0          (cells 0..15: a converging flow)
+#   eq (20)  vg_p = (v_{p-1} + 2 v_p + v_{p+1}) / 4:
+#     vg = 0 0 0 1/4 3/4 1 1 1/2 | -1/2 -1 -1 -3/4 -1/4 0 0 0   (cells 0..15)
+#   eq (22)  v_{7+1/2} = (vg_7 + vg_8)/2 = (1/2 - 1/2)/2 = 0 exactly, with vg_7 = -vg_8 != 0: THE TIE.
+#   eq (21), first-order fluxes f1 = vg B at faces 6.5, 7.5, 8.5:  1 (from cell 6),  vg_8 B_8 = -1/2 (tie: from cell 8,
+#     the "<= 0" arm; the "> 0" arm would give vg_7 B_7 = +1/2),  -1 (from cell 9)
+#   eq (16) half step  B' = B - (f1_{p+1/2} - f1_{p-1/2}) dt/2:   B'_6 = 1, B'_7 = 1 + 3/8 = 11/8, B'_8 = 1 + 1/8 = 9/8,
+#     B'_9 = 1, B'_5 = B'_10 = 15/16
+#   w = vg B':  w_5 = 15/16, w_6 = 1, w_7 = 11/16, w_8 = -9/16, w_9 = -1, w_10 = -15/16
+#   second-order fluxes (eqs (11)-(15) with the van Leer limiter 2ab/(a+b), zero when a b <= 0):
+#     face 6.5 (v > 0):  w_6 + vl((w_6 - w_5)/2, (w_7 - w_6)/2) = 1 + vl(1/32, -5/32) = 1
+#     face 8.5 (v < 0):  w_9 + vl((w_9 - w_10)/2, (w_8 - w_9)/2) = -1 + vl(-1/32, 7/32) = -1
+#     face 7.5 (tie, the arm of cell 8):  w_8 + vl((w_8 - w_9)/2, (w_7 - w_8)/2) = -9/16 + vl(7/32, 5/8)
+#                                         = -9/16 + 2 (7/32)(5/8) / (27/32) = -9/16 + 35/108 = -103/432
+#   eq (17)  B_7 = 1 - (-103/432 - 1)/2 = 1399/864,   B_8 = 1 - (-1 + 103/432)/2 = 1193/864.
+# With the tie sent to cell 7 instead ("v >= 0") the mirror image comes out: B_7 = 1193/864, B_8 = 1399/864.
+# ---------------------------------------------------------------------------------------------------------------
+TIE_V = [0, 0, 0, 0, 1, 1, 1, 1, -1, -1, -1, -1, 0, 0, 0, 0]
+TIE_B7, TIE_B8 = 1399.0 / 864.0, 1193.0 / 864.0
+
+
+def tie_state(d, t, shape3, dtype=np.float64, offset=0):
+    """the worked example laid along axis d (0 = x) of a grid of extents shape3 = (nx, ny, nz), uniform across the
+    pencils, the 16 cells starting at `offset` along d (zeros around them)"""
+    nx, ny, nz = shape3
+    sh = (nz, ny, nx)
+    nd = shape3[d]
+    v = np.zeros(nd)
+    v[offset:offset + 16] = TIE_V
+    bshape = [1, 1, 1]
+    bshape[2 - d] = nd
+    f = [np.ones(sh)] + [np.zeros(sh) for _ in range(3)] + [np.full(sh, 4.0)] + [np.zeros(sh) for _ in range(3)]
+    f[1 + d] = f[1 + d] + v.reshape(bshape)
+    f[5 + t] = f[5 + t] + 1.0
+    return [np.ascontiguousarray(a, dtype=dtype) for a in f]
+
+
+@pytest.mark.parametrize("d,t", [(0, 1), (0, 2), (1, 2), (1, 0), (2, 0), (2, 1)])
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-15), (np.float32, 3e-7)])
+def test_upwind_tie_takes_the_cell_on_the_right(d, t, dtype, tol):
+    shape3 = [1, 1, 1]
+    shape3[d] = 16
+    f = tie_state(d, t, shape3, dtype)
+    oracle.badvect(f, 5.0 / 3.0, P, d, t, 0.5)
+    b = f[5 + t].astype(np.float64).ravel()
+    assert abs(b[7] - TIE_B7) <= tol * TIE_B7, (b[7], TIE_B7)
+    assert abs(b[8] - TIE_B8) <= tol * TIE_B8, (b[8], TIE_B8)
+    assert b[7] > b[8] + 0.2                                  # the asymmetry IS the rule: "<= 0" sends the tie to cell i+1
+    assert abs(b.sum() - 16.0) <= 16 * tol                   # flux form: B_t is conserved along the pencil
+    for c in range(5, 8):                                    # nothing else moves
+        if c != 5 + t:
+            assert not f[c].any()
+    assert np.array_equal(f[0], np.ones_like(f[0])) and np.array_equal(f[4], np.full_like(f[4], 4.0))
