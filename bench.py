@@ -278,20 +278,30 @@ def main():
     roofline, breakdown = None, None
     if rank == 0 and not args.no_breakdown:
         dtv, _ = sol.cfl_dt(CFL)
+        # algorithmic words per cell of each row follow the PATH THAT RAN, read off the kernel launches one apply makes
+        # (ADVICE r2): a fluid kernel moves 13 words (8 in, 5 out), a B pair 8 (rho, m_d, 3 B in; 3 B out), a kernel that
+        # fuses B pair + fluid 16, one that fuses two B pairs 8; mhd_apply adds one 1-thread launch that sets dt
+        WORDS_BY_LAUNCHES = {"lrev": {1: (16, "one fused kernel"), 2: (8 + 13, "B pair kernel + fluid kernel")},
+                             "mid": {2: (13 + 16, "fluid kernel + one kernel fusing B pair, B pair, fluid"),
+                                     3: (13 + 8 + 13, "fluid + one kernel fusing the two B pairs + fluid"),
+                                     4: (13 + 8 + 8 + 13, "fluid, B pair, B pair, fluid: four kernels")}}
         kinds = [("fluid_x", B.MHD_OP_FLUID, 0, 13), ("fluid_y", B.MHD_OP_FLUID, 1, 13), ("fluid_z", B.MHD_OP_FLUID, 2, 13),
                  ("bpair_x", B.MHD_OP_BPAIR, 0, 8), ("bpair_y", B.MHD_OP_BPAIR, 1, 8), ("bpair_z", B.MHD_OP_BPAIR, 2, 8),
-                 ("lrev_x", B.MHD_OP_SWEEP_REVERSE, 0, 16),   # reverse L_x: one fused kernel (fp32) or B pair + fluid
-                 # reverse L_y / L_z: one kernel (B pair -> fluid through shared memory); middle pair of a step:
-                 # fluid kernel + one kernel for B pair, B pair, fluid (13 + 16 words)
-                 ("lrev_y", B.MHD_OP_SWEEP_REVERSE, 1, 16), ("lrev_z", B.MHD_OP_SWEEP_REVERSE, 2, 16),
-                 ("mid_y", B.MHD_OP_MIDDLE_PAIR, 1, 29), ("mid_z", B.MHD_OP_MIDDLE_PAIR, 2, 29)]
+                 ("lrev_x", B.MHD_OP_SWEEP_REVERSE, 0, "lrev"), ("lrev_y", B.MHD_OP_SWEEP_REVERSE, 1, "lrev"),
+                 ("lrev_z", B.MHD_OP_SWEEP_REVERSE, 2, "lrev"),
+                 ("mid_y", B.MHD_OP_MIDDLE_PAIR, 1, "mid"), ("mid_z", B.MHD_OP_MIDDLE_PAIR, 2, "mid")]
         breakdown = {}
         reps = 5
         with torch.cuda.stream(stream):
             for name, op, d, words in kinds:
                 sol.set_state(state)                           # repeated single operators are not a stable scheme: start each kind
                 dtv, _ = sol.cfl_dt(CFL)                       # from the workload's initial state, dt at its CFL limit
+                l0 = sol.launch_count()
                 sol.apply(op, d, 0, dtv)                       # warm
+                nk = sol.launch_count() - l0 - 1               # kernels of one apply, without the 1-thread set_dt launch
+                path = None
+                if isinstance(words, str):
+                    words, path = WORDS_BY_LAUNCHES[words].get(nk, (None, f"{nk} kernels"))
                 a, b = ev(), ev()
                 torch.cuda.synchronize()
                 a.record(stream)
@@ -300,7 +310,10 @@ def main():
                 b.record(stream)
                 torch.cuda.synchronize()
                 kms = a.elapsed_time(b) / reps                 # includes the 1-thread set_dt launch (~2 us)
-                breakdown[name] = {"ms": kms, "algo_GBps": words * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": words}
+                breakdown[name] = {"ms": kms, "algo_GBps": (words * esize * N / (kms * 1e-3) / 1e9) if words else None,
+                                   "words_per_cell": words, "kernels_per_apply": nk}
+                if path:
+                    breakdown[name]["path"] = path
             # the stand-alone c_max pass (first step / after mhd_apply only; steps fuse it into their last kernel):
             # cmax_reuse = 0 makes every mhd_cfl_dt run the reduction instead of returning the cached c_max
             sol.set_state(state)
@@ -315,7 +328,8 @@ def main():
             torch.cuda.synchronize()
             sol.set_option("cmax_reuse", 1)
             kms = a.elapsed_time(b) / reps             # includes the D2H read of dt and its synchronisation
-            breakdown["cfl"] = {"ms": kms, "algo_GBps": 8 * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": 8}
+            breakdown["cfl"] = {"ms": kms, "algo_GBps": 8 * esize * N / (kms * 1e-3) / 1e9, "words_per_cell": 8,
+                                "includes": "per call: the reduction kernel, the 1-thread dt kernel, the D2H read of dt and the stream synchronisation mhd_cfl_dt does (a step pays none of this: its reduction is fused into its last kernel)"}
         # Dominant kernel = largest share of a step.  Launches per step, averaged over the three sweep orders:
         # fluid_y, fluid_z 2 each (one kernel template, fluid_yz_ring_kernel, 4 launches), B pair y/z 2 each
         # (bpair_ring_kernel, 4 launches), fluid_x 1 + bpair_x 1 (forward L_x) and the reverse L_x (1).
@@ -330,7 +344,19 @@ def main():
         else:
             kms, words = breakdown[dom]["ms"], breakdown[dom]["words_per_cell"]
         ach = words * esize * N / (kms * 1e-3) / 1e9
+        # DRAM bytes one step actually moves (ncu dram__bytes of every kernel x its launches per step, profiles/r02_traffic.json)
+        # over the measured step time: the "achieved HBM GB/s" north_star's >= 60 % target is worded on
+        lpstep = {"fluid_yz": 4, "bpair_yz": 4, "fluid_x": 1, "bpair_x": 1, "lrev_x": 1}
+        tr = {k: ncu_traffic(args.workload, k) for k in lpstep}
+        if all(v is not None for v in tr.values()) and sol.launch_count() > 0 and breakdown["lrev_x"]["kernels_per_apply"] == 1:
+            dram_step = float(sum(tr[k] * lpstep[k] for k in lpstep))
+        elif all(tr.get(k) is not None for k in ("fluid_yz", "bpair_yz", "fluid_x", "bpair_x")):
+            dram_step = float(tr["fluid_yz"] * 4 + tr["bpair_yz"] * 4 + tr["fluid_x"] * 2 + tr["bpair_x"] * 2)   # reverse L_x as two kernels
+        else:
+            dram_step = None
+        step_s = (ms / args.steps) * 1e-3
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "frac_is": f"the dominant kernel ({dom}) alone on its own {words} words per cell; the whole step is roofline.step",
                     "traffic": ncu_traffic(args.workload, dom), "peak_source": peak_src,
                     "frac_of_spec_peak": ach / SPEC_PEAK_GBS,
                     "algorithmic_bytes_per_launch": words * esize * N, "ms_per_launch": kms,
@@ -338,7 +364,12 @@ def main():
                     "step": {"algorithmic_bytes_per_cell_step": ALGO_WORDS_STEP * esize,
                              "achieved": ALGO_WORDS_STEP * esize * (value / world) / 1e9,
                              "frac": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / peak,
-                             "frac_of_spec_peak": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / SPEC_PEAK_GBS}}
+                             "frac_of_spec_peak": ALGO_WORDS_STEP * esize * (value / world) / 1e9 / SPEC_PEAK_GBS,
+                             "dram_bytes_per_step_ncu": dram_step,
+                             "dram_gbs_achieved": (dram_step / step_s / 1e9) if dram_step else None,
+                             "dram_frac_of_measured_peak": (dram_step / step_s / 1e9 / peak) if dram_step else None,
+                             "dram_frac_of_spec_peak": (dram_step / step_s / 1e9 / SPEC_PEAK_GBS) if dram_step else None,
+                             "dram_source": "profiles/r02_traffic.json (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch) x launches per step / the step time measured here"}}
 
     # ---- end to end through the C ABI with HOST buffers ----------------------------------------
     e2e = None
@@ -470,8 +501,28 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": l2_note(8 * N * esize),
                        "t_grid_after": t_now},
-            "clocks": clocks, "gpu_launches": launches, "long_run": long_run, "others": others, "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
-            "kernels": breakdown,
+            "clocks": clocks, "gpu_launches": launches, "kernels": breakdown, "others": others, "e2e": e2e,
+            "roofline": roofline, "cpu_baseline": cpu, "long_run": long_run,
+        }
+        # LAST in the line, compact: the whole of BASELINE.json's metric ("fp32 & fp64 at 256^3/512^3") in one place, so
+        # that a record which keeps only the tail of the line still carries it
+        def brief(r):
+            return None if not r else {"steps": r["steps"], "ms_per_step": round(r["ms_per_step"], 4), "value": round(r["value"]),
+                                       "step_frac_of_measured_peak": round(r["roofline_step_frac"], 4),
+                                       "step_frac_of_spec_peak": round(r["roofline_step_frac_of_spec_peak"], 4),
+                                       "sm_mhz": (r.get("clocks") or {}).get("sm_mhz"), "reasons": (r.get("clocks") or {}).get("reasons")}
+        out["summary"] = {
+            "unit": "cell-updates/s; fractions are 96 words per cell-step (384 B fp32, 768 B fp64) x value over the HBM peak (measured copy rate / 8 TB/s data sheet)",
+            f"{args.workload}_at_--steps": {"steps": args.steps, "ms_per_step": round(ms / args.steps, 4), "value": round(value),
+                                           "step_frac_of_measured_peak": roofline and round(roofline["step"]["frac"], 4),
+                                           "step_frac_of_spec_peak": roofline and round(roofline["step"]["frac_of_spec_peak"], 4),
+                                           "dram_gbs_achieved": roofline and roofline["step"]["dram_gbs_achieved"] and round(roofline["step"]["dram_gbs_achieved"], 1),
+                                           "dram_frac_of_spec_peak": roofline and roofline["step"]["dram_frac_of_spec_peak"] and round(roofline["step"]["dram_frac_of_spec_peak"], 4),
+                                           "sm_mhz": clocks.get("sm_mhz") if clocks else None},
+            f"{args.workload}_at_config_steps": brief(long_run),
+            "c5_512^3_f64": brief((others or {}).get("c5")), "c3_256^3_f32": brief((others or {}).get("c3")),
+            "dominant_kernel_frac": roofline and round(roofline["frac"], 4),
+            "cpu_oracle_sample": cpu and cpu.get("sample"),
         }
         print(json.dumps(out))
     if sol is not None:
